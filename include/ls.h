@@ -1,0 +1,146 @@
+/*
+ * ls.h — C ABI of the B200-native floating-mean Lomb-Scargle hot path (libls_b200.so).
+ *
+ * What the library computes (citations: PAPER.md = /root/reference/PAPER.md of arXiv:2409.08090;
+ * north_star = BASELINE.json "north_star"; readings A1..A17 = DESIGN.md §3):
+ *
+ *   For each series b of a batch sharing one time array t[Nd] (batched mode) the
+ *   standard-normalised, weighted, floating-mean Lomb-Scargle power at f_k = f0 + k df,
+ *   k = 0..Nf-1 (Eq. 1; A1), obtained from the six trigonometric sums
+ *       Sh,Ch = sum_j h_j {sin,cos}(2 pi f_k t_j)     h_j = w_j (y_j - ybar_w)
+ *       S ,C  = sum_j w_j {sin,cos}(2 pi f_k t_j)     w_j = dy_j^-2 / sum dy^-2
+ *       S2,C2 = sum_j w_j {sin,cos}(4 pi f_k t_j)
+ *   which are the real/imaginary parts of three type-1 (non-uniform -> uniform) NUFFTs
+ *   (PAPER.md:24-27 Eq. 2, :45): strengths pre-multiplied by e^{2 pi i f_c t_j}
+ *   (f_c = f0 + floor(Nf/2) df; A4), spread onto a fine grid of n ~ sigma Nf cells with the
+ *   "exponential of semicircle" kernel, one equispaced FFT (cuFFT), diagonal
+ *   rescaling, then the tau / YY,YC,YS,CC,SS assembly named by north_star.
+ *
+ * Every step runs in hand-written sm_100a kernels (stats, bin-count + scan, premultiply-scatter,
+ * tile-owner spread, deconvolve + assemble) around one cuFFT plan.  There is NO CPU fallback:
+ * every entry point fails with LS_ERR_CUDA when no device is usable.
+ *
+ * Conventions
+ *   - All functions return an int status (LS_OK == 0); nothing throws, prints or exits.
+ *   - Pointers passed to ls_execute are DEVICE pointers; to ls_execute_host they are HOST
+ *     pointers.  The caller owns them; the library never frees or writes inputs.
+ *   - Layouts (row-major, contiguous):  t[Nd] (always double);  y[batch][Nd], power[batch][Nf]
+ *     in `dtype`;  dy[Nd] (shared by the batch) or dy[batch][Nd] when opts.dy_per_series.
+ *     power[b][k] is the periodogram of series b at f0 + k*df.
+ *   - ls_execute only ENQUEUES work on `cuda_stream` (a cudaStream_t; NULL = legacy default
+ *     stream) and returns; it performs no device synchronisation.  One execute may be in flight
+ *     per plan (plan-owned scratch); use one plan per stream for concurrency.
+ *   - dy_j <= 0 or non-finite inputs give undefined (NaN-propagating) output; there is no
+ *     device-side validation on the hot path.
+ */
+#ifndef LS_B200_H
+#define LS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ls_plan_s* ls_plan_t;            /* opaque; owns cuFFT plan, tables, scratch */
+
+enum { LS_F32 = 0, LS_F64 = 1 };                /* dtype of y, dy, power, fine grid and FFT (A9:
+                                                   t, grid coordinates, phase reduction and the
+                                                   assembly are fp64 for both) */
+enum {
+    LS_OK = 0,
+    LS_ERR_INVALID_VALUE = 1,   /* bad argument (see ls_plan) */
+    LS_ERR_ALLOC = 2,           /* host or device allocation failed */
+    LS_ERR_CUDA = 3,            /* CUDA runtime error, or no usable device */
+    LS_ERR_CUFFT = 4,           /* cuFFT error */
+    LS_ERR_UNSUPPORTED = 5,     /* size outside what the kernels index (n >= 2^31) */
+    LS_ERR_NOT_READY = 6        /* information requested before it exists */
+};
+
+/* Stage indices for ls_get_stage_ms (CUDA-event timings of the last execute when opts.timing). */
+enum {
+    LS_STAGE_STATS = 0,         /* K1  weights, weighted mean                                    */
+    LS_STAGE_SORT = 1,          /* K3  bin count + scan (both point sets)                        */
+    LS_STAGE_PREMUL = 2,        /* K2  time-rescale, phase premultiply, scatter to bin order, YY */
+    LS_STAGE_SPREAD = 3,        /* K4  tile-owner spreading of all M grids                       */
+    LS_STAGE_FFT = 4,           /* F   cuFFT (library; reported separately, north_star)          */
+    LS_STAGE_ASSEMBLE = 5,      /* K5+K6 mode extraction, deconvolution, tau + power assembly    */
+    LS_STAGE_TOTAL = 6,         /* whole execute                                                 */
+    LS_NUM_STAGES = 7
+};
+
+/* Optional tuning; a zero-initialised struct (or NULL) selects the defaults. */
+typedef struct {
+    int dy_per_series;      /* 0: dy[Nd] shared by the batch (A13, default); 1: dy[batch][Nd]     */
+    double upsampfac;       /* sigma; 0 = auto (2.0)                                              */
+    int kernel_width;       /* w in fine-grid cells; 0 = auto from eps (A10)                      */
+    int timing;             /* 1: record CUDA events around each stage of every execute           */
+    int device;             /* CUDA device ordinal the plan lives on                              */
+    int tile_cells;         /* spreading tile length L in cells; 0 = auto                         */
+    int batch_chunk;        /* transforms spread/FFT'd/assembled per pass; 0 = auto (L2-sized)    */
+    int reserved[8];        /* must be zero                                                       */
+} ls_opts;
+
+/* ls_plan — choose (sigma, w, beta, n) from eps ("width and fine grid size are
+ * carefully chosen to match the user tolerance"; A10), build the deconvolution table
+ * 1/psihat(k') ("diagonal rescaling"), the cuFFT plan and all scratch buffers.
+ *   Nd >= 1 points, Nf >= 1 frequencies, f0 >= 0 and df > 0 finite (cycles per unit of t),
+ *   eps in [1e-14, 1e-1] for LS_F64 / [1e-6, 1e-1] for LS_F32, batch >= 1.
+ * Errors: LS_ERR_INVALID_VALUE for anything outside those ranges or out == NULL;
+ * LS_ERR_UNSUPPORTED if the fine grid needs n >= 2^31 cells; LS_ERR_ALLOC / _CUDA / _CUFFT. */
+int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double eps,
+            int dtype, int batch, const ls_opts* opts /* NULL ok */);
+
+/* ls_execute — one pass of the whole hot path (§8(a) K1..K6 + cuFFT) for `batch` series.
+ *   t      device, const double[Nd]
+ *   y      device, const dtype[batch][Nd]
+ *   dy     device, const dtype[Nd] (or [batch][Nd] with opts.dy_per_series)
+ *   power  device, dtype[batch][Nf]   (written)
+ *   cuda_stream  cudaStream_t to enqueue on.
+ * Asynchronous; errors of earlier asynchronous work may surface here as LS_ERR_CUDA. */
+int ls_execute(ls_plan_t plan, const void* t, const void* y, const void* dy, void* power,
+               void* cuda_stream);
+
+/* ls_execute_host — the same with HOST buffers: copies t, y, dy to plan-owned device staging
+ * buffers, executes, copies power back and synchronises the stream before returning.  Pinned
+ * host memory makes the copies asynchronous with respect to each other, pageable memory works. */
+int ls_execute_host(ls_plan_t plan, const void* t, const void* y, const void* dy, void* power,
+                    void* cuda_stream);
+
+/* Parameters the plan chose.  Any out-pointer may be NULL.
+ *   sigma = n/Nf realised, w = kernel width, beta = ES shape parameter, n = fine-grid cells,
+ *   M = transforms per execute (batch + 2 with shared dy; 3*batch with per-series dy),
+ *   model_bytes = algorithmic HBM bytes per execute excluding the FFT. */
+int ls_get_info(ls_plan_t plan, double* sigma, int* w, double* beta, int64_t* n, int* M,
+                double* model_bytes);
+
+/* Device bytes the plan allocated (grids + cuFFT work area + tables + scratch). */
+size_t ls_workspace_bytes(ls_plan_t plan);
+
+/* Milliseconds per stage of the most recent execute (needs opts.timing = 1; synchronises on the
+ * recorded events).  ms[LS_NUM_STAGES]; n_stages entries are written.  LS_ERR_NOT_READY if no
+ * timed execute has run. */
+int ls_get_stage_ms(ls_plan_t plan, float* ms, int n_stages);
+
+/* Number of kernels (own + cuFFT exec calls) one ls_execute enqueues: own_kernels counts the
+ * library's own __global__ launches, fft_execs the cufftExec calls. */
+int ls_get_launch_counts(ls_plan_t plan, int* own_kernels, int* fft_execs);
+
+/* Test hooks: read intermediates of the most recent execute (synchronises the device).
+ *   ls_debug_modes: the deconvolved NUFFT outputs g_k of series `series` at the K indices
+ *     kidx[] (host) -> out[K][6] (host, double) = (Sh, Ch, S, C, S2, C2) as the assembly saw them.
+ *     Only valid when the plan runs the batch in one pass (batch_chunk >= M) .
+ *   ls_debug_stats: out[3*batch] (host) = (W, ybar, YY) per series. */
+int ls_debug_modes(ls_plan_t plan, int series, int64_t K, const int64_t* kidx, double* out);
+int ls_debug_stats(ls_plan_t plan, double* out);
+
+const char* ls_strerror(int code);
+
+/* Frees everything the plan allocated.  NULL is accepted. */
+int ls_destroy(ls_plan_t plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LS_B200_H */

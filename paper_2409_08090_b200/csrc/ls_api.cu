@@ -1,0 +1,530 @@
+// ls_api.cu — the C-ABI boundary (include/ls.h): plan construction, the execute sequence,
+// host-buffer execute, introspection.  Host logic only; every arithmetic step of the hot path
+// runs in the kernels of ls_pre.cu / ls_spread.cu / ls_post.cu and in one cuFFT plan.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "ls_internal.h"
+
+using lsb::dd;
+
+namespace {
+
+struct Pass {
+    int s0, C;          // series [s0, s0 + C)
+    int fft_slot0, fft_batch;
+};
+
+inline size_t real_bytes(int dtype) { return dtype == LS_F64 ? 8 : 4; }
+
+// exact product of an integer-valued double and a double as a double-double
+inline dd two_prod(double a, double b) {
+    dd r;
+    r.hi = a * b;
+    r.lo = fma(a, b, -r.hi);
+    return r;
+}
+// double-double + double (Knuth two-sum, then renormalise)
+inline dd dd_add_d(dd a, double b) {
+    const double s = a.hi + b;
+    const double bb = s - a.hi;
+    const double e = (a.hi - (s - bb)) + (b - bb);
+    const double lo = e + a.lo;
+    dd r;
+    r.hi = s + lo;
+    r.lo = lo - (r.hi - s);
+    return r;
+}
+
+// smallest even integer >= lo whose prime factors are all in {2, 3, 5}
+int64_t next_smooth_even(int64_t lo) {
+    if (lo < 2) lo = 2;
+    for (int64_t m = lo + (lo & 1);; m += 2) {
+        int64_t r = m;
+        while (r % 2 == 0) r /= 2;
+        while (r % 3 == 0) r /= 3;
+        while (r % 5 == 0) r /= 5;
+        if (r == 1) return m;
+    }
+}
+
+// Gauss-Legendre nodes/weights on [0, 1] (Newton on P_Q in long double).
+void gauss_legendre_01(int Q, double* z, double* wt) {
+    for (int i = 0; i < Q; ++i) {
+        long double x = cosl(3.14159265358979323846264338327950288L * (i + 0.75L) / (Q + 0.5L));
+        long double dp = 1;
+        for (int it = 0; it < 100; ++it) {
+            long double p0 = 1, p1 = x;
+            for (int k = 2; k <= Q; ++k) {
+                const long double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) / k;
+                p0 = p1;
+                p1 = p2;
+            }
+            dp = Q * (x * p1 - p0) / (x * x - 1);
+            const long double dx = p1 / dp;
+            x -= dx;
+            if (fabsl(dx) < 1e-19L) break;
+        }
+        // recompute derivative at the converged root
+        long double p0 = 1, p1 = x;
+        for (int k = 2; k <= Q; ++k) {
+            const long double p2 = ((2 * k - 1) * x * p1 - (k - 1) * p0) / k;
+            p0 = p1;
+            p1 = p2;
+        }
+        dp = Q * (x * p1 - p0) / (x * x - 1);
+        const long double wx = 2 / ((1 - x * x) * dp * dp);
+        z[i] = (double)((x + 1) / 2);
+        wt[i] = (double)(wx / 2);
+    }
+}
+
+template <typename T>
+cudaError_t dmalloc(ls_plan_s* p, T** ptr, size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    cudaError_t e = cudaMalloc((void**)ptr, bytes);
+    if (e == cudaSuccess) p->total_bytes += bytes;
+    return e;
+}
+
+void build_passes(const ls_plan_s* p, std::vector<Pass>& out) {
+    out.clear();
+    const bool per = p->opts.dy_per_series != 0;
+    for (int s0 = 0; s0 < p->batch; s0 += p->chunk) {
+        Pass ps;
+        ps.s0 = s0;
+        ps.C = std::min(p->chunk, p->batch - s0);
+        if (per) { ps.fft_slot0 = 0; ps.fft_batch = 3 * ps.C; }
+        else if (s0 == 0) { ps.fft_slot0 = 0; ps.fft_batch = 2 + ps.C; }
+        else { ps.fft_slot0 = 2; ps.fft_batch = ps.C; }
+        out.push_back(ps);
+    }
+}
+
+struct FftPlans {
+    int batch[3];
+    cufftHandle h[3];
+    int count;
+};
+
+cufftHandle find_fft(const ls_plan_s* p, int batch) {
+    if (p->has_first && p->first_batch == batch) return p->fft_first;
+    if (p->has_rem && p->rem_batch == batch) return p->fft_rem;
+    return p->fft_chunk;
+}
+
+int make_fft(ls_plan_s* p, cufftHandle* h, int batch, size_t* work) {
+    if (cufftCreate(h) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+    if (cufftSetAutoAllocation(*h, 0) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+    long long nn[1] = {(long long)p->n};
+    size_t ws = 0;
+    const cufftType type = p->dtype == LS_F64 ? CUFFT_Z2Z : CUFFT_C2C;
+    if (cufftMakePlanMany64(*h, 1, nn, nullptr, 1, p->n, nullptr, 1, p->n, type, batch, &ws) != CUFFT_SUCCESS)
+        return LS_ERR_CUFFT;
+    *work = std::max(*work, ws);
+    return LS_OK;
+}
+
+void stage_begin(ls_plan_s* p, int stage, cudaStream_t s) {
+    if (!p->opts.timing) return;
+    if (p->events_used == p->events.size()) {
+        lsb::StageEvent ev;
+        ev.stage = stage;
+        cudaEventCreate(&ev.beg);
+        cudaEventCreate(&ev.end);
+        p->events.push_back(ev);
+    }
+    p->events[p->events_used].stage = stage;
+    cudaEventRecord(p->events[p->events_used].beg, s);
+}
+void stage_end(ls_plan_s* p, cudaStream_t s) {
+    if (!p->opts.timing) return;
+    cudaEventRecord(p->events[p->events_used].end, s);
+    ++p->events_used;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ls_strerror(int code) {
+    switch (code) {
+        case LS_OK: return "success";
+        case LS_ERR_INVALID_VALUE: return "invalid argument";
+        case LS_ERR_ALLOC: return "allocation failed";
+        case LS_ERR_CUDA: return "CUDA error or no usable device";
+        case LS_ERR_CUFFT: return "cuFFT error";
+        case LS_ERR_UNSUPPORTED: return "problem size not supported";
+        case LS_ERR_NOT_READY: return "requested information is not available yet";
+        default: return "unknown error code";
+    }
+}
+
+int ls_destroy(ls_plan_t p) {
+    if (!p) return LS_OK;
+    if (p->has_first) cufftDestroy(p->fft_first);
+    if (p->has_chunk) cufftDestroy(p->fft_chunk);
+    if (p->has_rem) cufftDestroy(p->fft_rem);
+    cudaFree(p->fft_work);
+    cudaFree(p->grids);
+    cudaFree(p->dinv);
+    cudaFree(p->sums);
+    cudaFree(p->scan_tmp);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(p->ps[i].hist);
+        cudaFree(p->ps[i].bin_start);
+        cudaFree(p->ps[i].pos);
+        cudaFree(p->ps[i].l0);
+        cudaFree(p->ps[i].x0);
+        cudaFree(p->ps[i].q);
+        cudaFree(p->ps[i].rows);
+    }
+    cudaFree(p->st_t);
+    cudaFree(p->st_y);
+    cudaFree(p->st_dy);
+    cudaFree(p->st_p);
+    for (auto& ev : p->events) {
+        cudaEventDestroy(ev.beg);
+        cudaEventDestroy(ev.end);
+    }
+    delete p;
+    return LS_OK;
+}
+
+int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double eps, int dtype, int batch,
+            const ls_opts* opts) {
+    if (!out) return LS_ERR_INVALID_VALUE;
+    *out = nullptr;
+    if (Nd < 1 || Nf < 1 || batch < 1 || batch > 65535) return LS_ERR_INVALID_VALUE;
+    if (!(df > 0.0) || !isfinite(df) || !(f0 >= 0.0) || !isfinite(f0)) return LS_ERR_INVALID_VALUE;
+    if (dtype != LS_F32 && dtype != LS_F64) return LS_ERR_INVALID_VALUE;
+    const double eps_lo = dtype == LS_F64 ? 1e-14 : 1e-6;
+    if (!(eps >= eps_lo) || !(eps <= 1e-1)) return LS_ERR_INVALID_VALUE;
+    if (Nd >= (int64_t)1 << 31) return LS_ERR_UNSUPPORTED;
+    ls_opts o;
+    memset(&o, 0, sizeof o);
+    if (opts) o = *opts;
+    if (o.upsampfac != 0.0 && !(o.upsampfac >= 1.2 && o.upsampfac <= 4.0)) return LS_ERR_INVALID_VALUE;
+    if (o.kernel_width != 0 && (o.kernel_width < 2 || o.kernel_width > lsb::kMaxWidth)) return LS_ERR_INVALID_VALUE;
+    if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
+                              o.tile_cells > lsb::kSpreadThreads * 4))
+        return LS_ERR_INVALID_VALUE;
+    if (o.batch_chunk < 0) return LS_ERR_INVALID_VALUE;
+
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || o.device < 0 || o.device >= ndev) return LS_ERR_CUDA;
+    if (cudaSetDevice(o.device) != cudaSuccess) return LS_ERR_CUDA;
+
+    ls_plan_s* p = new (std::nothrow) ls_plan_s;
+    if (!p) return LS_ERR_ALLOC;
+    p->Nd = Nd; p->Nf = Nf; p->f0 = f0; p->df = df; p->eps = eps; p->dtype = dtype; p->batch = batch;
+    p->opts = o;
+
+    // ---- (sigma, w, beta, n) from eps: reading A10; two (fp64) / one (fp32) widths of safety so that a
+    // pointwise reading of the tolerance also holds (A8, A9).
+    p->sigma = o.upsampfac != 0.0 ? o.upsampfac : 2.0;
+    int w = o.kernel_width;
+    if (w == 0) {
+        if (p->sigma == 2.0) w = (int)ceil(log10(1.0 / eps) - 1e-12) + 1;
+        else w = (int)ceil(-log(eps) / (M_PI * sqrt(1.0 - 1.0 / p->sigma)));
+        w += dtype == LS_F64 ? 2 : 1;
+        w = std::max(2, std::min(lsb::kMaxWidth, w));
+    }
+    p->w = w;
+    p->beta = p->sigma == 2.0 ? 2.30 * w : 0.97 * M_PI * w * (1.0 - 1.0 / (2.0 * p->sigma));
+    const double want = ceil(p->sigma * (double)Nf);
+    if (want >= 2147483000.0) { delete p; return LS_ERR_UNSUPPORTED; }
+    p->n = next_smooth_even(std::max<int64_t>((int64_t)want, 2 * w));
+    if (p->n >= ((int64_t)1 << 31) - 4096) { delete p; return LS_ERR_UNSUPPORTED; }
+    p->L = o.tile_cells ? o.tile_cells : 1024;
+    p->nbins = (int)((p->n + lsb::kBinCells - 1) / lsb::kBinCells);
+    p->ntiles = (int)((p->n + p->L - 1) / p->L);
+    const bool per = o.dy_per_series != 0;
+    p->M = per ? 3 * batch : batch + 2;
+    const size_t B = real_bytes(dtype);
+    const size_t grid_bytes = (size_t)p->n * 2 * B;
+    if (o.batch_chunk > 0) p->chunk = std::min(o.batch_chunk, batch);
+    else p->chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)batch, ((size_t)64 << 20) / grid_bytes));
+    p->slots = per ? 3 * p->chunk : 2 + p->chunk;
+
+    // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
+    p->ndf = two_prod((double)p->n, df);
+    p->fc = dd_add_d(two_prod((double)(Nf / 2), df), f0);
+
+    p->model_bytes = 8.0 * Nd + (double)batch * Nd * B + (per ? (double)batch : 1.0) * Nd * B + 8.0 * Nd +
+                     (double)p->M * p->n * 2 * B + (double)p->M * Nf * 2 * B + (double)batch * Nf * B;
+
+    int rc = LS_OK;
+    cudaError_t ce = cudaSuccess;
+    do {
+        if ((ce = dmalloc(p, &p->grids, (size_t)p->slots * grid_bytes)) != cudaSuccess) break;
+        if ((ce = dmalloc(p, &p->dinv, (size_t)(Nf / 2 + 1) * 8)) != cudaSuccess) break;
+        if ((ce = dmalloc(p, &p->sums, (size_t)batch * 4 * 8)) != cudaSuccess) break;
+        const int nchunks = (p->nbins + 4095) / 4096;
+        if ((ce = dmalloc(p, &p->scan_tmp, (size_t)2 * (nchunks + 1) * 4)) != cudaSuccess) break;
+        if ((ce = cudaMemset(p->scan_tmp, 0, (size_t)2 * (nchunks + 1) * 4)) != cudaSuccess) break;
+        // both histograms live in ONE allocation so a single memset clears them
+        if ((ce = dmalloc(p, &p->ps[0].hist, (size_t)2 * p->nbins * 4)) != cudaSuccess) break;
+        p->ps[1].hist = p->ps[0].hist + p->nbins;
+        for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
+            lsb::PointSet& ps = p->ps[i];
+            ps.nrows = i == 0 ? (per ? 2 * batch : batch + 1) : (per ? batch : 1);
+            if ((ce = dmalloc(p, &ps.bin_start, (size_t)(p->nbins + 1) * 4)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, &ps.pos, (size_t)Nd * 4)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, &ps.l0, (size_t)Nd * 4)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, (char**)&ps.x0, (size_t)Nd * B)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, (char**)&ps.q, (size_t)Nd * 2 * B)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, (char**)&ps.rows, (size_t)ps.nrows * Nd * B)) != cudaSuccess) break;
+        }
+        if (ce != cudaSuccess) break;
+
+        // cuFFT plans for every distinct batch size the pass list needs, one shared work area
+        std::vector<Pass> passes;
+        build_passes(p, passes);
+        size_t work = 0;
+        p->first_batch = passes.front().fft_batch;
+        if ((rc = make_fft(p, &p->fft_first, p->first_batch, &work)) != LS_OK) break;
+        p->has_first = true;
+        if (passes.size() > 1) {
+            const int cb = passes[1].fft_batch;
+            if (cb != p->first_batch) {
+                if ((rc = make_fft(p, &p->fft_chunk, cb, &work)) != LS_OK) break;
+                p->has_chunk = true;
+            } else p->fft_chunk = p->fft_first;
+            const int rb = passes.back().fft_batch;
+            if (rb != cb && rb != p->first_batch) {
+                p->rem_batch = rb;
+                if ((rc = make_fft(p, &p->fft_rem, rb, &work)) != LS_OK) break;
+                p->has_rem = true;
+            }
+        } else p->fft_chunk = p->fft_first;
+        p->fft_work_bytes = work;
+        if ((ce = dmalloc(p, (char**)&p->fft_work, work)) != cudaSuccess) break;
+        if (cufftSetWorkArea(p->fft_first, p->fft_work) != CUFFT_SUCCESS) { rc = LS_ERR_CUFFT; break; }
+        if (p->has_chunk && cufftSetWorkArea(p->fft_chunk, p->fft_work) != CUFFT_SUCCESS) { rc = LS_ERR_CUFFT; break; }
+        if (p->has_rem && cufftSetWorkArea(p->fft_rem, p->fft_work) != CUFFT_SUCCESS) { rc = LS_ERR_CUFFT; break; }
+
+        // P0: deconvolution table on the device
+        double hz[lsb::kQuadNodes], hw[lsb::kQuadNodes];
+        gauss_legendre_01(lsb::kQuadNodes, hz, hw);
+        double* dq = nullptr;
+        if ((ce = cudaMalloc((void**)&dq, sizeof(double) * 2 * lsb::kQuadNodes)) != cudaSuccess) break;
+        ce = cudaMemcpy(dq, hz, sizeof hz, cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess) ce = cudaMemcpy(dq + lsb::kQuadNodes, hw, sizeof hw, cudaMemcpyHostToDevice);
+        if (ce == cudaSuccess) ce = lsb::launch_deconv_table(p, dq, dq + lsb::kQuadNodes, 0);
+        if (ce == cudaSuccess) ce = cudaDeviceSynchronize();
+        cudaFree(dq);
+    } while (0);
+    if (ce != cudaSuccess) rc = (ce == cudaErrorMemoryAllocation) ? LS_ERR_ALLOC : LS_ERR_CUDA;
+    if (rc != LS_OK) {
+        cudaGetLastError();
+        ls_destroy(p);
+        return rc;
+    }
+    *out = p;
+    return LS_OK;
+}
+
+int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, void* cuda_stream) {
+    if (!p || !t || !y || !dy || !power) return LS_ERR_INVALID_VALUE;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const bool per = p->opts.dy_per_series != 0;
+    int own = 0, ffts = 0;
+    cudaError_t ce = cudaSuccess;
+    p->events_used = 0;
+#define LS_TRY(call)                 \
+    do {                             \
+        ce = (call);                 \
+        if (ce != cudaSuccess) {     \
+            cudaGetLastError();      \
+            return LS_ERR_CUDA;      \
+        }                            \
+    } while (0)
+
+    stage_begin(p, LS_STAGE_TOTAL, s);
+    const size_t total_slot = p->events_used;   // the TOTAL event pair is closed at the very end
+    if (p->opts.timing) ++p->events_used;
+
+    stage_begin(p, LS_STAGE_STATS, s);
+    LS_TRY(cudaMemsetAsync(p->sums, 0, (size_t)p->batch * 4 * 8, s));
+    LS_TRY(lsb::launch_stats(p, (const double*)t, y, dy, s)); ++own;
+    stage_end(p, s);
+
+    stage_begin(p, LS_STAGE_SORT, s);
+    LS_TRY(cudaMemsetAsync(p->ps[0].hist, 0, (size_t)2 * p->nbins * 4, s));
+    LS_TRY(lsb::launch_bin_count(p, (const double*)t, s)); ++own;
+    LS_TRY(lsb::launch_bin_scan(p, s)); own += 2;
+    stage_end(p, s);
+
+    stage_begin(p, LS_STAGE_PREMUL, s);
+    LS_TRY(lsb::launch_premultiply(p, (const double*)t, s)); ++own;
+    LS_TRY(lsb::launch_rows(p, y, dy, s)); ++own;
+    stage_end(p, s);
+
+    {
+        std::vector<Pass> passes;
+        build_passes(p, passes);
+        for (const Pass& ps : passes) {
+            int h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride;
+            stage_begin(p, LS_STAGE_SPREAD, s);
+            if (per) {
+                // slots [0, C): w2_s ; slots [C, 3C): (w_s, h_s) pairs
+                LS_TRY(lsb::launch_spread(p, 1, ps.s0, ps.C, 0, s)); ++own;
+                LS_TRY(lsb::launch_spread(p, 0, 2 * ps.s0, 2 * ps.C, ps.C, s)); ++own;
+                w2_slot = 0; w2_stride = 1; w_slot = ps.C; w_stride = 2; h_slot = ps.C + 1; h_stride = 2;
+            } else {
+                // slot 0: w2, slot 1: w, slots 2..: h_s of this pass
+                if (ps.s0 == 0) {
+                    LS_TRY(lsb::launch_spread(p, 1, 0, 1, 0, s)); ++own;
+                    LS_TRY(lsb::launch_spread(p, 0, 0, 1 + ps.C, 1, s)); ++own;
+                } else {
+                    LS_TRY(lsb::launch_spread(p, 0, 1 + ps.s0, ps.C, 2, s)); ++own;
+                }
+                w2_slot = 0; w2_stride = 0; w_slot = 1; w_stride = 0; h_slot = 2; h_stride = 1;
+            }
+            stage_end(p, s);
+
+            stage_begin(p, LS_STAGE_FFT, s);
+            {
+                cufftHandle h = find_fft(p, ps.fft_batch);
+                if (cufftSetStream(h, s) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+                char* base = (char*)p->grids + (size_t)ps.fft_slot0 * p->n * 2 * real_bytes(p->dtype);
+                // B_k = sum_l b_l e^{+2 pi i k l / n}  (reading A7)  ==  cuFFT's unnormalised inverse
+                cufftResult fr = p->dtype == LS_F64
+                                     ? cufftExecZ2Z(h, (cufftDoubleComplex*)base, (cufftDoubleComplex*)base, CUFFT_INVERSE)
+                                     : cufftExecC2C(h, (cufftComplex*)base, (cufftComplex*)base, CUFFT_INVERSE);
+                if (fr != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+                ++ffts;
+            }
+            stage_end(p, s);
+
+            stage_begin(p, LS_STAGE_ASSEMBLE, s);
+            LS_TRY(lsb::launch_assemble(p, ps.s0, ps.C, h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride, power, s));
+            ++own;
+            stage_end(p, s);
+        }
+    }
+    if (p->opts.timing) {
+        cudaEventRecord(p->events[total_slot].end, s);
+        p->timed_once = true;
+    }
+    p->own_kernels = own;
+    p->fft_execs = ffts;
+    return LS_OK;
+#undef LS_TRY
+}
+
+int ls_execute_host(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, void* cuda_stream) {
+    if (!p || !t || !y || !dy || !power) return LS_ERR_INVALID_VALUE;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const size_t B = real_bytes(p->dtype);
+    const size_t bt = (size_t)p->Nd * 8, by = (size_t)p->batch * p->Nd * B;
+    const size_t bdy = (size_t)(p->opts.dy_per_series ? p->batch : 1) * p->Nd * B;
+    const size_t bp = (size_t)p->batch * p->Nf * B;
+    if (!p->st_t) {
+        if (dmalloc(p, (char**)&p->st_t, bt) != cudaSuccess || dmalloc(p, (char**)&p->st_y, by) != cudaSuccess ||
+            dmalloc(p, (char**)&p->st_dy, bdy) != cudaSuccess || dmalloc(p, (char**)&p->st_p, bp) != cudaSuccess) {
+            cudaGetLastError();
+            return LS_ERR_ALLOC;
+        }
+    }
+    if (cudaMemcpyAsync(p->st_t, t, bt, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+        cudaMemcpyAsync(p->st_y, y, by, cudaMemcpyHostToDevice, s) != cudaSuccess ||
+        cudaMemcpyAsync(p->st_dy, dy, bdy, cudaMemcpyHostToDevice, s) != cudaSuccess) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    const int rc = ls_execute(p, p->st_t, p->st_y, p->st_dy, p->st_p, cuda_stream);
+    if (rc != LS_OK) return rc;
+    if (cudaMemcpyAsync(power, p->st_p, bp, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+        cudaStreamSynchronize(s) != cudaSuccess) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    return LS_OK;
+}
+
+int ls_get_info(ls_plan_t p, double* sigma, int* w, double* beta, int64_t* n, int* M, double* model_bytes) {
+    if (!p) return LS_ERR_INVALID_VALUE;
+    if (sigma) *sigma = (double)p->n / (double)p->Nf;
+    if (w) *w = p->w;
+    if (beta) *beta = p->beta;
+    if (n) *n = p->n;
+    if (M) *M = p->M;
+    if (model_bytes) *model_bytes = p->model_bytes;
+    return LS_OK;
+}
+
+size_t ls_workspace_bytes(ls_plan_t p) { return p ? p->total_bytes : 0; }
+
+int ls_get_stage_ms(ls_plan_t p, float* ms, int n_stages) {
+    if (!p || !ms || n_stages < 1) return LS_ERR_INVALID_VALUE;
+    if (!p->opts.timing || !p->timed_once) return LS_ERR_NOT_READY;
+    float acc[LS_NUM_STAGES] = {0};
+    for (size_t i = 0; i < p->events_used; ++i) {
+        const lsb::StageEvent& ev = p->events[i];
+        if (cudaEventSynchronize(ev.end) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+        float v = 0;
+        if (cudaEventElapsedTime(&v, ev.beg, ev.end) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+        acc[ev.stage] += v;
+    }
+    for (int i = 0; i < n_stages && i < LS_NUM_STAGES; ++i) ms[i] = acc[i];
+    return LS_OK;
+}
+
+int ls_get_launch_counts(ls_plan_t p, int* own_kernels, int* fft_execs) {
+    if (!p) return LS_ERR_INVALID_VALUE;
+    if (p->own_kernels == 0) return LS_ERR_NOT_READY;
+    if (own_kernels) *own_kernels = p->own_kernels;
+    if (fft_execs) *fft_execs = p->fft_execs;
+    return LS_OK;
+}
+
+int ls_debug_stats(ls_plan_t p, double* out) {
+    if (!p || !out) return LS_ERR_INVALID_VALUE;
+    std::vector<double> h((size_t)p->batch * 4);
+    if (cudaDeviceSynchronize() != cudaSuccess ||
+        cudaMemcpy(h.data(), p->sums, h.size() * 8, cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    const bool per = p->opts.dy_per_series != 0;
+    for (int s = 0; s < p->batch; ++s) {
+        const double W = h[per ? 4 * s : 0];
+        out[3 * s + 0] = W;
+        out[3 * s + 1] = h[4 * s + 1] / W;
+        out[3 * s + 2] = h[4 * s + 2];
+    }
+    return LS_OK;
+}
+
+int ls_debug_modes(ls_plan_t p, int series, int64_t K, const int64_t* kidx, double* out) {
+    if (!p || !kidx || !out || K < 1 || series < 0 || series >= p->batch) return LS_ERR_INVALID_VALUE;
+    if (p->chunk < p->batch) return LS_ERR_NOT_READY;          // grids of earlier passes are gone
+    for (int64_t i = 0; i < K; ++i)
+        if (kidx[i] < 0 || kidx[i] >= p->Nf) return LS_ERR_INVALID_VALUE;
+    const bool per = p->opts.dy_per_series != 0;
+    const int C = p->batch;
+    const int h_slot = per ? C + 2 * series + 1 : 2 + series;
+    const int w_slot = per ? C + 2 * series : 1;
+    const int w2_slot = per ? series : 0;
+    int64_t* dk = nullptr;
+    double* dout = nullptr;
+    int rc = LS_OK;
+    if (cudaMalloc((void**)&dk, K * 8) != cudaSuccess || cudaMalloc((void**)&dout, K * 48) != cudaSuccess) rc = LS_ERR_ALLOC;
+    if (rc == LS_OK && (cudaDeviceSynchronize() != cudaSuccess ||
+                        cudaMemcpy(dk, kidx, K * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
+                        lsb::launch_debug_modes(p, h_slot, w_slot, w2_slot, K, dk, dout, 0) != cudaSuccess ||
+                        cudaMemcpy(out, dout, K * 48, cudaMemcpyDeviceToHost) != cudaSuccess))
+        rc = LS_ERR_CUDA;
+    cudaFree(dk);
+    cudaFree(dout);
+    if (rc != LS_OK) cudaGetLastError();
+    return rc;
+}
+
+}  // extern "C"

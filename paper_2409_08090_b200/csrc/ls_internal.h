@@ -1,0 +1,101 @@
+// ls_internal.h — plan structure and kernel launchers shared by the library's translation units.
+// Internal to libls_b200.so; the public boundary is include/ls.h.  Nothing here is shared with
+// oracle/ (the CPU oracle is test infrastructure and has its own, independent arithmetic).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <cufft.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/ls.h"
+
+namespace lsb {
+
+constexpr int kMaxWidth = 16;        // widest spreading kernel supported (cells)
+constexpr int kBinCells = 256;       // sort-bin length Lb in fine-grid cells (>= kMaxWidth/2 + 1)
+constexpr int kSpreadThreads = 256;  // threads per spreading CTA
+constexpr int kQuadNodes = 64;       // Gauss-Legendre nodes on [0,1] for psihat
+
+// double-double constant (hi + lo), built on the host with FMA error-free products.
+struct dd {
+    double hi, lo;
+};
+
+// One non-uniform point set in bin-sorted order (x1 = n df t, or x2 = 2 x1).
+struct PointSet {
+    int* hist = nullptr;       // [nbins]   bin counts -> running cursors during the scatter
+    int* bin_start = nullptr;  // [nbins+1] exclusive scan of the counts
+    int* pos = nullptr;        // [Nd]      sorted slot of input point j
+    int* l0 = nullptr;         // [Nd]      first fine-grid cell touched (unfolded, may be <0 or >=n)
+    void* x0 = nullptr;        // [Nd] T    offset of that cell from the point, in [-w/2, -w/2+1)
+    void* q = nullptr;         // [Nd] T2   unit phasor e^{2 pi i f_c t} (x1) or its square (x2)
+    void* rows = nullptr;      // [nrows][Nd] T  real strengths per transform, sorted order
+    int nrows = 0;
+};
+
+struct StageEvent {
+    int stage;
+    cudaEvent_t beg, end;
+};
+
+}  // namespace lsb
+
+struct ls_plan_s {
+    // problem
+    int64_t Nd = 0, Nf = 0, n = 0;
+    double f0 = 0, df = 0, eps = 0;
+    int dtype = LS_F64, batch = 1;
+    ls_opts opts{};
+    // chosen parameters
+    double sigma = 2.0, beta = 0;
+    int w = 0;
+    int L = 1024;          // spreading tile length (cells), multiple of kBinCells
+    int nbins = 0;         // ceil(n / kBinCells)
+    int ntiles = 0;        // ceil(n / L)
+    int M = 0;             // transforms per execute
+    int chunk = 1;         // series per pass
+    int slots = 0;         // grid slots allocated
+    lsb::dd ndf{}, fc{};   // n*df and f_c = f0 + floor(Nf/2) df as double-doubles
+    // device buffers
+    void* grids = nullptr;      // [slots][n] complex T
+    double* dinv = nullptr;     // [floor(Nf/2)+1] 1/psihat(k')
+    double* sums = nullptr;     // [batch][4]  (sum dy^-2, sum dy^-2 y, YY, unused)
+    int* scan_tmp = nullptr;    // block sums + ticket for the bin scan (both point sets)
+    lsb::PointSet ps[2];
+    // host staging for ls_execute_host
+    void *st_t = nullptr, *st_y = nullptr, *st_dy = nullptr, *st_p = nullptr;
+    // cuFFT
+    cufftHandle fft_first = 0, fft_chunk = 0, fft_rem = 0;
+    bool has_first = false, has_chunk = false, has_rem = false;
+    int first_batch = 0, rem_batch = 0;
+    void* fft_work = nullptr;
+    size_t fft_work_bytes = 0;
+    size_t total_bytes = 0;
+    // timing
+    std::vector<lsb::StageEvent> events;
+    size_t events_used = 0;
+    bool timed_once = false;
+    int own_kernels = 0, fft_execs = 0;
+    double model_bytes = 0;
+};
+
+namespace lsb {
+
+// ---- ls_pre.cu: K1 stats, K3 bin count + scan, K2 premultiply + scatter --------------------
+cudaError_t launch_stats(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s);
+cudaError_t launch_bin_count(ls_plan_s* p, const double* t, cudaStream_t s);
+cudaError_t launch_bin_scan(ls_plan_s* p, cudaStream_t s);
+cudaError_t launch_premultiply(ls_plan_s* p, const double* t, cudaStream_t s);
+cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_t s);
+// ---- ls_spread.cu: K4 ----------------------------------------------------------------------
+cudaError_t launch_spread(ls_plan_s* p, int pointset, int row0, int nrows, int slot0, cudaStream_t s);
+// ---- ls_post.cu: P0 table, K5+K6 -----------------------------------------------------------
+cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double* weights, cudaStream_t s);
+cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,
+                            int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s);
+cudaError_t launch_debug_modes(ls_plan_s* p, int h_slot, int w_slot, int w2_slot, int64_t K,
+                               const int64_t* d_kidx, double* d_out, cudaStream_t s);
+
+}  // namespace lsb

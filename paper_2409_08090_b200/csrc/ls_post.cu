@@ -1,0 +1,165 @@
+// ls_post.cu — P0 deconvolution table, and K5+K6: mode extraction, diagonal rescaling
+// ("correct with a diagonal rescaling") fused with the tau / power assembly
+// (north_star: "compute tan(2 omega tau), then the YY/YC/YS/CC/SS terms and the
+// standard-normalised power").
+//
+// Mode k of the periodogram (f_k = f0 + k df) is the centred NUFFT mode k' = k - floor(Nf/2)
+// (Eq. 2; readings A2, A4), stored by the FFT at index k' mod n.  Re g = C, Im g = S
+// (A7).  The assembly runs in fp64 registers for both dtypes (A9).
+#include "ls_internal.h"
+
+namespace lsb {
+namespace {
+
+constexpr int kPostThreads = 256;
+
+// psihat(k') = (w/2) * int_{-1}^{1} phi(z) cos(pi w k' z / n) dz,  phi even -> twice the half range.
+// nodes/weights: Gauss-Legendre on [0, 1].
+__global__ void __launch_bounds__(kPostThreads)
+ls_deconv_table_kernel(double* __restrict__ dinv, long long count, const double* __restrict__ nodes,
+                       const double* __restrict__ weights, int w, double beta, double inv_n) {
+    __shared__ double sz[kQuadNodes], sf[kQuadNodes];
+    if (threadIdx.x < kQuadNodes) {
+        const double z = nodes[threadIdx.x];
+        sz[threadIdx.x] = z;
+        sf[threadIdx.x] = weights[threadIdx.x] * exp(beta * (sqrt(fmax(0.0, 1.0 - z * z)) - 1.0));
+    }
+    __syncthreads();
+    const long long k = (long long)blockIdx.x * kPostThreads + threadIdx.x;
+    if (k >= count) return;
+    const double a = (double)w * (double)k * inv_n;      // argument of cos(pi a z)
+    double acc = 0.0;
+#pragma unroll 4
+    for (int i = 0; i < kQuadNodes; ++i) acc = fma(sf[i], cospi(a * sz[i]), acc);
+    dinv[k] = 1.0 / ((double)w * acc);                   // (w/2) * 2 * sum
+}
+
+template <typename T>
+struct V2;
+template <>
+struct V2<double> { using type = double2; };
+template <>
+struct V2<float> { using type = float2; };
+
+struct AssembleArgs {
+    const void* grids;
+    long long n, Nf;
+    long long half;                 // floor(Nf/2)
+    const double* dinv;
+    const double* sums;
+    int series0, dy_per_series;
+    int h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride;
+    void* power;
+};
+
+// The assembly formulas exactly as north_star lists them, with
+//   C2w = |den|/r, S2w = num sign(den)/r, r = hypot(num, den)   [= 1/sqrt(1+tan^2), tan C2w]
+//   Sw  = S2w / (2 Cw)                                           [= sign(S2w) sqrt((1-C2w)/2)]
+// and the conventions of reading A14 for 0/0 and non-positive CC, SS.
+__device__ __forceinline__ double assemble_power(double Sh, double Ch, double S, double C, double S2, double C2,
+                                                 double inv_YY) {
+    const double num = S2 - 2.0 * S * C;
+    const double den = C2 - (C * C - S * S);
+    const double r = sqrt(num * num + den * den);
+    double C2w = 1.0, S2w = 0.0;
+    if (r > 0.0) {
+        const double ir = 1.0 / r;
+        C2w = fabs(den) * ir;
+        S2w = (den < 0.0 ? -num : num) * ir;
+    }
+    const double Cw = sqrt(0.5 * (1.0 + C2w));
+    const double Sw = S2w / (2.0 * Cw);
+    const double YC = Ch * Cw + Sh * Sw;
+    const double YS = Sh * Cw - Ch * Sw;
+    const double a = C * Cw + S * Sw, b = S * Cw - C * Sw;
+    const double CC = 0.5 * (1.0 + C2 * C2w + S2 * S2w) - a * a;
+    const double SS = 0.5 * (1.0 - C2 * C2w - S2 * S2w) - b * b;
+    double P = 0.0;
+    if (CC > 0.0) P += YC * YC / CC;
+    if (SS > 0.0) P += YS * YS / SS;
+    return P * inv_YY;
+}
+
+template <typename T>
+__global__ void __launch_bounds__(kPostThreads)
+ls_assemble_kernel(const AssembleArgs a) {
+    using T2 = typename V2<T>::type;
+    const long long k = (long long)blockIdx.x * kPostThreads + threadIdx.x;
+    if (k >= a.Nf) return;
+    const int i = blockIdx.y;                      // series within this pass
+    const int s = a.series0 + i;
+    const long long kp = k - a.half;               // centred mode k'
+    const long long idx = kp < 0 ? kp + a.n : kp;
+    const double d = a.dinv[kp < 0 ? -kp : kp];
+    const T2* g = reinterpret_cast<const T2*>(a.grids);
+    const T2 gh = __ldcs(&g[(long long)(a.h_slot + i * a.h_stride) * a.n + idx]);
+    const T2 gw = g[(long long)(a.w_slot + i * a.w_stride) * a.n + idx];
+    const T2 g2 = g[(long long)(a.w2_slot + i * a.w2_stride) * a.n + idx];
+    const double YY = a.sums[4 * s + 2];
+    const double P = assemble_power((double)gh.y * d, (double)gh.x * d, (double)gw.y * d, (double)gw.x * d,
+                                    (double)g2.y * d, (double)g2.x * d, 1.0 / YY);
+    reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k] = (T)P;
+}
+
+template <typename T>
+__global__ void ls_debug_modes_kernel(const void* grids, long long n, long long half, const double* dinv,
+                                      int h_slot, int w_slot, int w2_slot, long long K,
+                                      const long long* kidx, double* out) {
+    using T2 = typename V2<T>::type;
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= K) return;
+    const long long kp = kidx[q] - half;
+    const long long idx = kp < 0 ? kp + n : kp;
+    const double d = dinv[kp < 0 ? -kp : kp];
+    const T2* g = reinterpret_cast<const T2*>(grids);
+    const T2 gh = g[(long long)h_slot * n + idx], gw = g[(long long)w_slot * n + idx], g2 = g[(long long)w2_slot * n + idx];
+    double* o = out + 6 * q;
+    o[0] = (double)gh.y * d; o[1] = (double)gh.x * d;
+    o[2] = (double)gw.y * d; o[3] = (double)gw.x * d;
+    o[4] = (double)g2.y * d; o[5] = (double)g2.x * d;
+}
+
+}  // namespace
+
+cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double* weights, cudaStream_t s) {
+    const long long count = p->Nf / 2 + 1;
+    const int nb = (int)((count + kPostThreads - 1) / kPostThreads);
+    ls_deconv_table_kernel<<<nb, kPostThreads, 0, s>>>(p->dinv, count, nodes, weights, p->w, p->beta,
+                                                       1.0 / (double)p->n);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,
+                            int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s) {
+    AssembleArgs a;
+    a.grids = p->grids;
+    a.n = p->n;
+    a.Nf = p->Nf;
+    a.half = p->Nf / 2;
+    a.dinv = p->dinv;
+    a.sums = p->sums;
+    a.series0 = series0;
+    a.dy_per_series = p->opts.dy_per_series;
+    a.h_slot = h_slot; a.h_stride = h_stride;
+    a.w_slot = w_slot; a.w_stride = w_stride;
+    a.w2_slot = w2_slot; a.w2_stride = w2_stride;
+    a.power = power;
+    dim3 grid((unsigned)((p->Nf + kPostThreads - 1) / kPostThreads), nseries);
+    if (p->dtype == LS_F64) ls_assemble_kernel<double><<<grid, kPostThreads, 0, s>>>(a);
+    else ls_assemble_kernel<float><<<grid, kPostThreads, 0, s>>>(a);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_debug_modes(ls_plan_s* p, int h_slot, int w_slot, int w2_slot, int64_t K,
+                               const int64_t* d_kidx, double* d_out, cudaStream_t s) {
+    const int nb = (int)((K + 127) / 128);
+    if (p->dtype == LS_F64)
+        ls_debug_modes_kernel<double><<<nb, 128, 0, s>>>(p->grids, p->n, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
+                                                         K, (const long long*)d_kidx, d_out);
+    else
+        ls_debug_modes_kernel<float><<<nb, 128, 0, s>>>(p->grids, p->n, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
+                                                        K, (const long long*)d_kidx, d_out);
+    return cudaGetLastError();
+}
+
+}  // namespace lsb
