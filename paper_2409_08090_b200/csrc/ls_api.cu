@@ -174,8 +174,8 @@ int ls_destroy(ls_plan_t p) {
     cudaFree(p->dinv);
     cudaFree(p->sums);
     cudaFree(p->scan_tmp);
+    cudaFree(p->ps[0].hist);                 // ps[1].hist points into the same allocation
     for (int i = 0; i < 2; ++i) {
-        cudaFree(p->ps[i].hist);
         cudaFree(p->ps[i].bin_start);
         cudaFree(p->ps[i].pos);
         cudaFree(p->ps[i].l0);

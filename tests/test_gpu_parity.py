@@ -1,0 +1,292 @@
+"""-m gpu parity tests: the CUDA path (through the C-ABI binding) against the CPU oracle, element by
+element on the same seeded inputs.
+
+Gate (BASELINE.json north_star, reading A8): E_inf = max|P_gpu - P_or| / max P_or
+  <= 1e-8 (fp64, eps 1e-9)   <= 1e-4 (fp32, eps 1e-5).
+Pointwise statistics (the paper's metric) are asserted against the band the paper
+reports for nifty-ls itself (median <= 1e-8, 99th percentile <= 1e-6 in fp64).
+"""
+import numpy as np
+import pytest
+
+from gpu_util import GATE_F32, GATE_F64, errors, gpu_power, oracle_power
+from paper_2409_08090_b200.workloads import Workload, compare_indices, make_workload, scaled_workload
+
+pytestmark = pytest.mark.gpu
+
+
+def _custom(t, y, dy, f0, df, Nf, dtype="f64", eps=1e-9, name="custom"):
+    t = np.ascontiguousarray(t, dtype=np.float64)
+    npd = np.float64 if dtype == "f64" else np.float32
+    y = np.atleast_2d(np.asarray(y, dtype=npd))
+    dy = np.asarray(dy, dtype=npd)
+    return Workload(name, t, np.ascontiguousarray(y), np.ascontiguousarray(dy), float(f0), float(df), int(Nf), dtype, eps)
+
+
+def _check64(e, pointwise=True):
+    assert e["Einf"] <= GATE_F64, e
+    if pointwise:
+        assert e["median"] <= 1e-8 and e["p99"] <= 1e-6, e
+
+
+# ------------------------------------------------------------------ the five configs
+def test_cfg1_full_grid():
+    w = make_workload(1)
+    Pg, ex = gpu_power(w, return_plan_info=True)
+    Po = oracle_power(w)
+    e = errors(Pg[0], Po)
+    _check64(e)
+    assert int(np.argmax(Pg[0])) == int(np.argmax(Po))
+    assert ex["launches"][0] > 0 and ex["launches"][1] == 1            # our kernels ran; one cuFFT exec
+    assert ex["info"]["M"] == 3 and ex["info"]["n"] >= 2 * w.Nf - 2
+
+
+def test_cfg2_full_grid_unsorted_times():
+    w = make_workload(2)
+    Pg = gpu_power(w)
+    e = errors(Pg[0], oracle_power(w, fast=True))
+    _check64(e)
+    ks = compare_indices(w, 512)
+    _check64(errors(Pg[0][ks], oracle_power(w, ks=ks)), pointwise=False)   # strict direct evaluation on a subset
+
+
+def test_cfg3_headline_size_sampled_frequencies():
+    """Full size (N_d = 1e6, N_f = 1.25e7, n = 2.5e7) in the launch configuration bench.py times;
+    compared on sampled k the oracle evaluates one by one (seam, edges and the injected peak included)."""
+    w = make_workload(3)
+    Pg = gpu_power(w)
+    assert np.all(np.isfinite(Pg)) and Pg.min() >= -1e-12 and Pg.max() <= 1 + 1e-9
+    ks = compare_indices(w, 384)
+    Po = oracle_power(w, ks=ks)
+    e = errors(Pg[0][ks], Po)
+    _check64(e)
+    kpk = ks[np.argmax(Po)]
+    lo, hi = max(0, kpk - 50), min(w.Nf, kpk + 51)
+    assert lo + int(np.argmax(Pg[0][lo:hi])) == kpk
+
+
+def test_cfg3_time_shift_invariance_full_grid():
+    """A property that holds at any size (north_star: invariance of power to shifting t), on the FULL
+    grid of the headline config: P(t + Delta) == P(t) up to the perturbation rounding t + Delta makes."""
+    w = make_workload(3)
+    P0 = gpu_power(w)[0]
+    w2 = _custom(w.t + 4096.0, w.y, w.dy, w.f0, w.df, w.Nf)
+    P1 = gpu_power(w2)[0]
+    # fl(t + 4096) moves t by <= 2^-40 day; at f_max = 250/day that is a 2e-10-cycle phase change per point
+    assert np.max(np.abs(P1 - P0)) / P0.max() <= 1e-8
+
+
+def test_cfg4_scaled_batch_full_grid():
+    w = scaled_workload(4, 2000, batch=37)
+    Pg, ex = gpu_power(w, return_plan_info=True)
+    assert ex["info"]["M"] == 39
+    for b in (0, 1, 17, 36):
+        _check64(errors(Pg[b], oracle_power(w, b)))
+
+
+def test_cfg4_full_size_batch_1000():
+    w = make_workload(4)
+    Pg = gpu_power(w)
+    assert Pg.shape == (1000, 125_000) and np.all(np.isfinite(Pg))
+    ks = compare_indices(w, 48)[:96]
+    worst = 0.0
+    for b in range(w.batch):                                           # every series on a small subset
+        e = errors(Pg[b][ks], oracle_power(w, b, ks=ks))
+        worst = max(worst, e["Einf"])
+    assert worst <= GATE_F64, worst
+    ks = compare_indices(w, 1024)
+    for b in (0, 333, 999):                                            # a few series on a large subset
+        _check64(errors(Pg[b][ks], oracle_power(w, b, ks=ks)))
+
+
+def test_cfg5_scaled_fp32_clustered():
+    w = scaled_workload(5, 100_000)
+    Pg = gpu_power(w)
+    ks = compare_indices(w, 2048)
+    e = errors(Pg[0][ks], oracle_power(w, ks=ks))
+    assert e["Einf"] <= GATE_F32, e
+    assert e["median"] <= 1e-4, e
+
+
+def test_cfg5_full_size_fp32_sampled_frequencies():
+    w = make_workload(5)
+    Pg = gpu_power(w)
+    assert np.all(np.isfinite(Pg))
+    ks = compare_indices(w, 24)
+    e = errors(Pg[0][ks], oracle_power(w, ks=ks))
+    assert e["Einf"] <= GATE_F32, e
+
+
+# ------------------------------------------------------------------ stage pins (debug exports)
+def test_stats_and_nufft_contract():
+    """K1 against the oracle's statistics; the three type-1 transforms against the oracle's direct
+    sums: ||g~ - g||_2 / ||g||_2 <~ eps."""
+    import oracle
+    w = make_workload(2)
+    ks = compare_indices(w, 1500)
+    Pg, ex = gpu_power(w, return_plan_info=True, debug_modes=(0, ks))
+    W, ybar, YY = oracle.stats(w.y[0], w.dy)
+    assert abs(ex["stats"][0, 0] - W) <= 1e-12 * W
+    assert abs(ex["stats"][0, 1] - ybar) <= 1e-13
+    assert abs(ex["stats"][0, 2] - YY) <= 1e-12 * YY
+    _, sums, _ = oracle.direct(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, k=ks, return_sums=True)
+    g = ex["modes"]
+    for a, b in ((0, 1), (2, 3), (4, 5)):                              # (Sh,Ch), (S,C), (S2,C2)
+        num = np.sqrt(np.sum((g[:, a] - sums[:, a]) ** 2 + (g[:, b] - sums[:, b]) ** 2))
+        den = np.sqrt(np.sum(sums[:, a] ** 2 + sums[:, b] ** 2))
+        assert num / den <= w.eps, (a, num / den)
+
+
+# ------------------------------------------------------------------ options and layouts
+@pytest.mark.parametrize("opts", [dict(tile_cells=256), dict(tile_cells=512), dict(kernel_width=10),
+                                  dict(upsampfac=1.25), dict(kernel_width=16, upsampfac=1.25)])
+def test_plan_options(opts):
+    w = scaled_workload(2, 3000)
+    Pg = gpu_power(w, **opts)
+    e = errors(Pg[0], oracle_power(w, fast=True))
+    _check64(e, pointwise=False)
+
+
+def test_batch_chunking_matches_single_pass():
+    w = scaled_workload(4, 1500, batch=11)
+    P_one = gpu_power(w, batch_chunk=11)
+    for chunk in (1, 3, 4, 10):
+        P_c = gpu_power(w, batch_chunk=chunk)
+        assert np.max(np.abs(P_c - P_one)) <= 1e-12
+    for b in (0, 10):
+        _check64(errors(P_one[b], oracle_power(w, b)))
+
+
+def test_per_series_dy():
+    w = scaled_workload(4, 1200, batch=5)
+    rng = np.random.default_rng(7)
+    w.dy = np.ascontiguousarray(rng.uniform(0.5, 1.5, (5, w.Nd)))
+    for chunk in (0, 2):
+        Pg = gpu_power(w, batch_chunk=chunk)
+        for b in range(5):
+            _check64(errors(Pg[b], oracle_power(w, b)))
+
+
+def test_execute_host_matches_device():
+    w = scaled_workload(2, 2500)
+    Pd = gpu_power(w)
+    Ph = gpu_power(w, host=True)
+    assert np.max(np.abs(Pd - Ph)) <= 1e-12
+    w5 = scaled_workload(5, 30_000)
+    assert np.max(np.abs(gpu_power(w5) - gpu_power(w5, host=True))) <= 1e-5
+
+
+def test_repeat_execute_is_stable():
+    """Tile-owner spreading uses no floating-point atomics on the grid: repeated executes of one plan
+    agree to rounding of the (atomic) statistics sums."""
+    w = scaled_workload(3, 20_000)
+    a = gpu_power(w)
+    b = gpu_power(w)
+    assert np.max(np.abs(a - b)) <= 1e-13
+
+
+# ------------------------------------------------------------------ edge cases
+def test_periodic_wrap_when_points_exceed_the_period():
+    """df*T > 1/2: the x2 = 2 x1 point set (and here x1 too) wraps around the periodic fine grid (A6)."""
+    rng = np.random.default_rng(3)
+    Nd, Nf = 400, 700
+    t = rng.uniform(-50.0, 150.0, Nd)
+    y = np.sin(2 * np.pi * 0.31 * t) + rng.normal(0, 0.2, Nd)
+    dy = rng.uniform(0.5, 1.5, Nd)
+    w = _custom(t, y, dy, f0=0.05, df=0.0131, Nf=Nf)                   # df*T = 2.6 periods
+    _check64(errors(gpu_power(w)[0], oracle_power(w)), pointwise=False)
+
+
+@pytest.mark.parametrize("Nf", [1, 2, 3, 17, 1001])
+def test_small_and_odd_Nf(Nf):
+    rng = np.random.default_rng(100 + Nf)
+    Nd = 50
+    t = np.sort(rng.uniform(0, 20, Nd)); y = rng.normal(0, 1, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    w = _custom(t, y, dy, f0=0.02, df=0.011, Nf=Nf)
+    _check64(errors(gpu_power(w)[0], oracle_power(w)), pointwise=False)
+
+
+@pytest.mark.parametrize("Nd", [3, 4, 33, 257])
+def test_tiny_Nd(Nd):
+    rng = np.random.default_rng(Nd)
+    t = rng.uniform(0, 10, Nd); y = rng.normal(0, 1, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    w = _custom(t, y, dy, f0=0.013, df=0.017, Nf=200)
+    Pg, Po = gpu_power(w)[0], oracle_power(w)
+    if Nd == 3:
+        # 3 points, 3 parameters: the model interpolates, P = 1 wherever the fit is well-conditioned
+        good = np.abs(Po - 1) < 1e-9
+        assert good.sum() > 100 and np.max(np.abs(Pg[good] - 1)) < 1e-6
+    else:
+        assert np.max(np.abs(Pg - Po)) <= 1e-8
+
+
+def test_all_points_in_one_cell_and_duplicates():
+    """Degenerate clustering: every point inside one fine-grid cell (one sort bin takes everything)."""
+    rng = np.random.default_rng(9)
+    Nd = 5000
+    t = 100.0 + rng.uniform(0, 1e-7, Nd)
+    t[::7] = t[0]                                                     # exact duplicates
+    y = rng.normal(0, 1, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    w = _custom(t, y, dy, f0=0.01, df=0.01, Nf=300)
+    Pg, Po = gpu_power(w)[0], oracle_power(w)
+    assert np.all(np.isfinite(Pg))
+    # the periodogram of coincident points is ill-conditioned (CC*SS -> 0): compare where it is not
+    good = Po < 0.99
+    assert np.max(np.abs(Pg[good] - Po[good])) <= 1e-6 or good.sum() == 0
+
+
+def test_f0_zero_convention():
+    """f0 = 0: k = 0 is the zero frequency, where the sine term vanishes (reading A14: that term is
+    dropped, P = 0 — parity unpinned for that one value); every k >= 1 must match the oracle."""
+    rng = np.random.default_rng(12)
+    Nd = 300
+    t = rng.uniform(0, 50, Nd); y = rng.normal(1.0, 1, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    w = _custom(t, y, dy, f0=0.0, df=0.004, Nf=900)
+    Pg, Po = gpu_power(w)[0], oracle_power(w)
+    assert np.max(np.abs(Pg[1:] - Po[1:])) / Po[1:].max() <= GATE_F64
+    assert np.isfinite(Pg[0]) and abs(Pg[0]) <= 1e-6
+
+
+def test_noiseless_sinusoid_peaks_at_one():
+    rng = np.random.default_rng(41)
+    Nd, Nf = 3000, 20000
+    t = rng.uniform(0, 200, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min())); kg = 7777
+    y = 3.1 + 1.3 * np.sin(2 * np.pi * (df + kg * df) * t + 0.9)
+    Pg = gpu_power(_custom(t, y, dy, df, df, Nf))[0]
+    assert int(np.argmax(Pg)) == kg and abs(1.0 - Pg[kg]) <= 1e-8
+
+
+def test_dy_scale_invariance():
+    w = scaled_workload(2, 4000)
+    P0 = gpu_power(w)[0]
+    w2 = _custom(w.t, w.y, 4.0 * w.dy, w.f0, w.df, w.Nf)
+    assert np.max(np.abs(gpu_power(w2)[0] - P0)) <= 1e-12
+
+
+def test_invalid_arguments_are_rejected():
+    from gpu_util import require_cuda
+    require_cuda()
+    from paper_2409_08090_b200 import binding as B
+    bad = [dict(Nd=0), dict(Nf=0), dict(df=0.0), dict(df=float("nan")), dict(f0=-1.0), dict(eps=1e-16),
+           dict(eps=0.5), dict(dtype=7), dict(batch=0)]
+    base = dict(Nd=100, Nf=1000, f0=0.1, df=0.1, eps=1e-9, dtype=B.LS_F64, batch=1)
+    for b in bad:
+        kw = dict(base, **b)
+        with pytest.raises(B.LsError) as ei:
+            B.ls_plan(**kw)
+        assert ei.value.code == 1, (b, ei.value.code)
+    with pytest.raises(B.LsError) as ei:
+        B.ls_plan(100, 1000, 0.1, 0.1, 1e-7, B.LS_F32, 1)              # eps below the fp32 floor
+    assert ei.value.code == 1
+    with pytest.raises(B.LsError) as ei:
+        B.ls_plan(100, 2_000_000_000, 0.1, 0.1, 1e-9, B.LS_F64, 1)     # n >= 2^31
+    assert ei.value.code == 5
+    h = B.ls_plan(**base)
+    with pytest.raises(B.LsError):
+        B.ls_execute(h, 0, 0, 0, 0, 0)                                 # NULL buffers
+    with pytest.raises(B.LsError) as ei:
+        B.ls_get_stage_ms(h)                                           # timing not enabled
+    assert ei.value.code == 6
+    B.ls_destroy(h)
+    B.ls_destroy(None)                                                 # NULL accepted
