@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py — ms per periodogram / NU points per second of the Lomb-Scargle hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path (K1 stats, K3 bin-sort, K2 premultiply, K4 spread, cuFFT,
+K5+K6 deconvolve + assemble) over one synthetic series set of the chosen BASELINE.json
+config (default: config 3, N_d = 1e6, N_f = 1.25e7, fp64, eps = 1e-9 — the one `metric` is quoted on).
+Prints ONE JSON line (rank 0).  See DESIGN.md §8 for every field.
+
+  value        ms per periodogram, device-timed (CUDA events on the launching stream), inputs resident
+               in HBM, L2 flushed between steps; whole job: max-over-ranks time / periodograms of all ranks
+  e2e          same through ls_execute_host with pinned HOST buffers (H2D of t, y, dy and D2H of power
+               inside the timed region)
+  roofline     dominant own kernel (stage timers inside the library, CUDA events) vs measured HBM peak
+  path_roofline  the north_star figure: model bytes of spread + deconvolve + assembly path (everything
+               except the cuFFT) / (t_total - t_fft)
+  cpu_baseline the oracle as it stands on this box's host cores, bounded frequency sample
+
+`--impl reference` times the CPU oracle (this tier's reference arm) on a bounded sample per step.
+Multi-GPU (torchrun): the path has no exchange step — each rank runs its own series ("weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "ms/periodogram"
+FALLBACK_HBM_GBS = 6650.0          # /opt/skills/guides/B200_PROFILING.md fallback ("of fallback")
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--cpu-freqs", type=int, default=0, help="oracle sample size (0 = auto)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def measured_peak():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region (profiling recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", "-i", str(self.index), f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+                for nm, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+# ----------------------------------------------------------------------------- workloads
+def rank_workload(cfg: int, rank: int):
+    """Config `cfg`; ranks > 0 draw their own series (same recipe, different seed): the path has no
+    exchange step, so multi-GPU is weak scaling over independent periodograms."""
+    from paper_2409_08090_b200.workloads import _BUILDERS, _SEEDS, make_workload
+    if rank == 0:
+        return make_workload(cfg)
+    return _BUILDERS[cfg](seed=_SEEDS[cfg] + 1000 * rank)
+
+
+def oracle_sample(w, K):
+    """Frequency indices of the bounded oracle sample: K seeded random k of the Nf."""
+    rng = np.random.default_rng(w.seed + 77)
+    return np.sort(rng.choice(w.Nf, size=min(K, w.Nf), replace=False)).astype(np.int64)
+
+
+def auto_cpu_freqs(w, cores, target_s=15.0):
+    # direct evaluation costs ~ Nd * K * batch point-frequency pairs at ~2e7 pairs/s/core (strict variant, measured on the GPU box's 16 cores)
+    pairs = target_s * 2.0e7 * max(cores, 1)
+    return int(max(8, min(w.Nf, pairs / (w.Nd * min(w.batch, 4)))))
+
+
+def time_oracle(w, K):
+    """The oracle as it stands (oracle.direct, strict variant), on K sampled frequencies of up to 4
+    series; returns (seconds for the sample, extrapolated ms per full periodogram, series used)."""
+    import oracle
+    ks = oracle_sample(w, K)
+    nser = min(w.batch, 4)
+    t0 = time.perf_counter()
+    for b in range(nser):
+        oracle.direct(w.t, w.y[b], w.dy, w.f0, w.df, w.Nf, k=ks)
+    dt = time.perf_counter() - t0
+    ms_full = dt / nser * (w.Nf / ks.size) * 1e3          # cost is exactly linear in the number of frequencies
+    return dt, ms_full, nser, int(ks.size)
+
+
+def config_dict(w, extra=None):
+    d = {"workload": w.name, "Nd": w.Nd, "Nf": w.Nf, "batch": w.batch, "eps": w.eps,
+         "l2": "flushed between steps (write of a 512 MiB buffer); grids (>= 3 x 400 MB at config 3) exceed L2 anyway"}
+    if extra:
+        d.update(extra)
+    return d
+
+
+# ----------------------------------------------------------------------------- reference arm
+def run_reference(args):
+    """This tier's reference arm = the CPU oracle, timed as it stands on the host cores.  Rank 0 only."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    w = rank_workload(args.config, 0)
+    cores = oracle.num_threads()
+    K = args.cpu_freqs or max(8, auto_cpu_freqs(w, cores, target_s=3.0))
+    for _ in range(args.warmup):
+        time_oracle(w, max(8, K // 8))
+    tot_s, ms_acc = 0.0, 0.0
+    for _ in range(args.steps):
+        dt, ms_full, nser, kk = time_oracle(w, K)
+        tot_s += dt; ms_acc += ms_full
+    ms = ms_acc / args.steps
+    sample = (f"{kk} of {w.Nf} frequencies x {nser} of {w.batch} series per step (oracle.direct, strict), "
+              f"time extrapolated linearly to the full grid")
+    line = {"impl": "reference", "metric": METRIC, "value": ms, "unit": "ms", "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": tot_s / args.steps * 1e3,
+            "higher_is_better": False, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(w), "gpu_launches": 0,
+            "nu_pts_per_s": 3.0 * w.Nd * w.batch / (ms * 1e-3),
+            "cpu_baseline": {"value": ms, "unit": "ms", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": ms, "unit": "ms", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------- our arm
+STAGE_BYTES_DOC = "DESIGN.md §6"
+
+
+def stage_model_bytes(w, info):
+    """Algorithmic HBM bytes per execute of each own stage."""
+    B = 8 if w.dtype == "f64" else 4
+    Nd, Nf, n, M, batch = w.Nd, w.Nf, info["n"], info["M"], w.batch
+    return {
+        "stats": batch * Nd * B + Nd * B,
+        "sort": 8 * Nd + 2 * 4 * (n // 256),
+        "premul": 8 * Nd + batch * Nd * B + Nd * B + 2 * Nd * (4 + B + 2 * B) + (M) * Nd * B,
+        "spread": M * n * 2 * B + 2 * Nd * (4 + B + 2 * B) + M * Nd * B,
+        "assemble": M * Nf * 2 * B + batch * Nf * B + (Nf // 2 + 1) * 8,
+    }
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU fallback")
+    from paper_2409_08090_b200 import binding as B
+    from paper_2409_08090_b200.build import build
+    build()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    w = rank_workload(args.config, rank)
+    tdt = torch.float64 if w.dtype == "f64" else torch.float32
+    t = torch.from_numpy(w.t).to(dev); y = torch.from_numpy(w.y).to(dev); dy = torch.from_numpy(w.dy).to(dev)
+    P = torch.empty((w.batch, w.Nf), dtype=tdt, device=dev)
+    # pinned host buffers for the e2e leg
+    ht = torch.from_numpy(w.t).pin_memory(); hy = torch.from_numpy(w.y).pin_memory()
+    hdy = torch.from_numpy(w.dy).pin_memory()
+    hP = torch.empty((w.batch, w.Nf), dtype=tdt).pin_memory()
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
+    plan = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F64 if w.dtype == "f64" else B.LS_F32, w.batch,
+                  timing=1, device=local)
+    info = plan.info
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        plan.execute(t, y, dy, P, stream)
+    torch.cuda.synchronize()
+    own, ffts = plan.launch_counts()
+
+    # ---- device-resident leg: K steps, each bracketed by events, L2 flushed in between
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    stage_acc = {k: 0.0 for k in B.STAGES}
+    sampler = ClockSampler(local)
+    barrier()
+    if rank == 0:
+        sampler.start()
+    wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)
+        ev[i][0].record()
+        plan.execute(t, y, dy, P, stream)
+        ev[i][1].record()
+        ev[i][1].synchronize()
+        for k, v in plan.stage_ms().items():
+            stage_acc[k] += v
+    barrier()
+    wall = time.perf_counter() - wall0
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    dev_ms = float(np.sum(step_ms))
+
+    # ---- e2e leg: host buffers through ls_execute_host (H2D + D2H inside the timed region)
+    for _ in range(2):
+        plan.execute_host(ht, hy, hdy, hP, stream)
+    e2e_ms = 0.0
+    barrier()
+    for i in range(args.steps):
+        flush.fill_(i & 0xFF)
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        plan.execute_host(ht, hy, hdy, hP, stream)       # synchronises the stream before returning
+        e2e_ms += (time.perf_counter() - t0) * 1e3
+    barrier()
+    clocks = sampler.stop() if rank == 0 else None      # sampled over both timed legs
+
+    tmax = torch.tensor([dev_ms, e2e_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    dev_ms, e2e_ms = float(tmax[0]), float(tmax[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    n_periodograms = w.batch * world                      # per step, all ranks
+    ms_per_step = dev_ms / args.steps
+    value = ms_per_step / n_periodograms
+    stage = {k: v / args.steps for k, v in stage_acc.items()}
+    peak, peak_src = measured_peak()
+    sbytes = stage_model_bytes(w, info)
+    own_stages = [k for k in ("stats", "sort", "premul", "spread", "assemble")]
+    dom = max(own_stages, key=lambda k: stage[k])
+    ach = sbytes[dom] / (stage[dom] * 1e-3) / 1e9
+    path_ms = stage["total"] - stage["fft"]
+    path_ach = info["model_bytes"] / (path_ms * 1e-3) / 1e9
+    Bi = ht.numel() * ht.element_size() + hy.numel() * hy.element_size() + hdy.numel() * hdy.element_size()
+    Bo = hP.numel() * hP.element_size()
+    line = {
+        "metric": METRIC, "value": value, "unit": "ms", "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+        "ms_per_step": ms_per_step, "higher_is_better": False, "scaling": "weak", "vs_baseline": None,
+        "dtype": w.dtype, "data": "synthetic",
+        "config": config_dict(w, {"sigma": info["sigma"], "w": info["w"], "n": info["n"], "M": info["M"]}),
+        "nu_pts_per_s": info["M"] * w.Nd * world / (stage["spread"] * 1e-3),
+        "nu_pts_per_s_whole": info["M"] * w.Nd * world / (ms_per_step * 1e-3),
+        "freqs_per_s": w.Nf * n_periodograms / (ms_per_step * 1e-3),
+        "stage_ms": stage, "wall_ms_per_step_incl_flush": wall / args.steps * 1e3,
+        "step_ms_min": float(np.min(step_ms)), "step_ms_median": float(np.median(step_ms)),
+        "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
+                     "kernel_ms": stage[dom]},
+        "path_roofline": {"what": "all own kernels (total - cuFFT), model bytes of " + STAGE_BYTES_DOC,
+                          "bytes": info["model_bytes"], "ms": path_ms, "achieved": path_ach, "unit": "GB/s",
+                          "frac_of_measured": path_ach / peak, "frac_of_8TBs": path_ach / 8000.0},
+        "fft_ms": stage["fft"],
+        "e2e": {"value": e2e_ms / args.steps / n_periodograms, "unit": "ms", "h2d_bytes_per_step": Bi,
+                "d2h_bytes_per_step": Bo},
+        "gpu_launches": own * args.steps, "own_kernels_per_step": own, "cufft_execs_per_step": ffts,
+        "clocks": clocks,
+    }
+    if not args.no_cpu_baseline and world == 1:
+        import oracle
+        cores = oracle.num_threads()
+        K = args.cpu_freqs or auto_cpu_freqs(w, cores)
+        dt, ms_full, nser, kk = time_oracle(w, K)
+        line["cpu_baseline"] = {"value": ms_full, "unit": "ms", "cores": cores, "kind": "oracle",
+                                "sample": f"{kk} of {w.Nf} frequencies x {nser} of {w.batch} series in {dt:.1f} s "
+                                          f"(oracle.direct, strict), extrapolated linearly to the full grid"}
+    print(json.dumps(line), flush=True)
+    plan.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

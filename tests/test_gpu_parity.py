@@ -206,33 +206,53 @@ def test_small_and_odd_Nf(Nf):
     _check64(errors(gpu_power(w)[0], oracle_power(w)), pointwise=False)
 
 
+def _sums_close(w, tol):
+    """The three transforms themselves (well-conditioned even when the power is not), against the
+    NUFFT contract |g~_k - g_k| <= tol * sum_j |c_j| (eps is relative to the strengths)."""
+    import oracle
+    ks = np.arange(w.Nf)
+    _, ex = gpu_power(w, debug_modes=(0, ks))
+    _, sums, _ = oracle.direct(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, return_sums=True)
+    wn = w.dy.astype(np.float64) ** -2.0
+    wn /= wn.sum()
+    l1_h = np.sum(np.abs(wn * (w.y[0] - np.sum(wn * w.y[0]))))           # sum |h_j|; sum |w_j| = 1
+    scale = np.array([l1_h, l1_h, 1.0, 1.0, 1.0, 1.0])
+    assert np.max(np.abs(ex["modes"] - sums) / scale) <= tol
+
+
 @pytest.mark.parametrize("Nd", [3, 4, 33, 257])
 def test_tiny_Nd(Nd):
     rng = np.random.default_rng(Nd)
     t = rng.uniform(0, 10, Nd); y = rng.normal(0, 1, Nd); dy = rng.uniform(0.5, 1.5, Nd)
     w = _custom(t, y, dy, f0=0.013, df=0.017, Nf=200)
     Pg, Po = gpu_power(w)[0], oracle_power(w)
+    _sums_close(w, 1e-9)
     if Nd == 3:
-        # 3 points, 3 parameters: the model interpolates, P = 1 wherever the fit is well-conditioned
+        # 3 points, 3 parameters: the model interpolates, P = 1; CC, SS are differences of O(1) numbers
+        # that nearly cancel, which amplifies the NUFFT's 1e-12 error in the sums (ill-conditioned)
         good = np.abs(Po - 1) < 1e-9
-        assert good.sum() > 100 and np.max(np.abs(Pg[good] - 1)) < 1e-6
+        assert good.sum() > 100 and np.max(np.abs(Pg[good] - 1)) < 1e-4
+        assert np.median(np.abs(Pg[good] - 1)) < 1e-8
+    elif Nd == 4:
+        # one degree of freedom left: still close to singular at some frequencies
+        assert np.max(np.abs(Pg - Po)) <= 1e-6 and np.median(np.abs(Pg - Po)) <= 1e-9
     else:
         assert np.max(np.abs(Pg - Po)) <= 1e-8
 
 
 def test_all_points_in_one_cell_and_duplicates():
-    """Degenerate clustering: every point inside one fine-grid cell (one sort bin takes everything)."""
+    """Degenerate clustering: every point inside one fine-grid cell (one sort bin takes everything).
+    All phases coincide to 1e-9 cycle, so CC*SS - CS^2 -> 0 and the POWER is ill-conditioned at any
+    precision; what the kernels must get right here are the transforms, which are compared tightly."""
     rng = np.random.default_rng(9)
     Nd = 5000
     t = 100.0 + rng.uniform(0, 1e-7, Nd)
     t[::7] = t[0]                                                     # exact duplicates
     y = rng.normal(0, 1, Nd); dy = rng.uniform(0.5, 1.5, Nd)
     w = _custom(t, y, dy, f0=0.01, df=0.01, Nf=300)
-    Pg, Po = gpu_power(w)[0], oracle_power(w)
+    Pg = gpu_power(w)[0]
     assert np.all(np.isfinite(Pg))
-    # the periodogram of coincident points is ill-conditioned (CC*SS -> 0): compare where it is not
-    good = Po < 0.99
-    assert np.max(np.abs(Pg[good] - Po[good])) <= 1e-6 or good.sum() == 0
+    _sums_close(w, 1e-9)
 
 
 def test_f0_zero_convention():
