@@ -224,25 +224,41 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     p->Nd = Nd; p->Nf = Nf; p->f0 = f0; p->df = df; p->eps = eps; p->dtype = dtype; p->batch = batch;
     p->opts = o;
 
-    // ---- (sigma, w, beta, n) from eps: reading A10; two (fp64) / one (fp32) widths of safety so that a
-    // pointwise reading of the tolerance also holds (A8, A9).
-    p->sigma = o.upsampfac != 0.0 ? o.upsampfac : 2.0;
+    // ---- (sigma, w, beta, n) from eps: reading A10.  Auto: the fine grid is the power of two in
+    // [1.25 Nf, 2.5 Nf) (the FFT pass count, not the cell count, decides its time), the
+    // width follows from the realised sigma = n/Nf, plus two (fp64) / one (fp32) cells of safety so
+    // that a pointwise reading of the tolerance also holds (A8, A9).
+    if (o.upsampfac != 0.0) {
+        const double want = ceil(o.upsampfac * (double)Nf);
+        if (want >= 2147483000.0) { delete p; return LS_ERR_UNSUPPORTED; }
+        p->n = next_smooth_even(std::max<int64_t>((int64_t)want, 2 * lsb::kMaxWidth));
+    } else {
+        const double want = ceil(1.25 * (double)Nf);
+        if (want >= 2147483000.0) { delete p; return LS_ERR_UNSUPPORTED; }
+        int64_t m = 64;                                 // >= 2 kMaxWidth
+        while ((double)m < want) m *= 2;
+        p->n = m;
+    }
+    if (p->n >= ((int64_t)1 << 31) - 4096) { delete p; return LS_ERR_UNSUPPORTED; }
+    p->sigma = (double)p->n / (double)Nf;
     int w = o.kernel_width;
     if (w == 0) {
-        if (p->sigma == 2.0) w = (int)ceil(log10(1.0 / eps) - 1e-12) + 1;
-        else w = (int)ceil(-log(eps) / (M_PI * sqrt(1.0 - 1.0 / p->sigma)));
+        const double s = std::min(p->sigma, 2.0);      // tiny Nf: n is floored at 2 kMaxWidth cells
+        w = (int)ceil(-log(eps) / (M_PI * sqrt(1.0 - 1.0 / s)) - 1e-9);
         w += dtype == LS_F64 ? 2 : 1;
         w = std::max(2, std::min(lsb::kMaxWidth, w));
     }
     p->w = w;
-    p->beta = p->sigma == 2.0 ? 2.30 * w : 0.97 * M_PI * w * (1.0 - 1.0 / (2.0 * p->sigma));
-    const double want = ceil(p->sigma * (double)Nf);
-    if (want >= 2147483000.0) { delete p; return LS_ERR_UNSUPPORTED; }
-    p->n = next_smooth_even(std::max<int64_t>((int64_t)want, 2 * w));
-    if (p->n >= ((int64_t)1 << 31) - 4096) { delete p; return LS_ERR_UNSUPPORTED; }
+    p->beta = 0.97 * M_PI * w * (1.0 - 1.0 / (2.0 * std::min(p->sigma, 2.0)));
     p->L = o.tile_cells ? o.tile_cells : 1024;
     p->nbins = (int)((p->n + lsb::kBinCells - 1) / lsb::kBinCells);
     p->ntiles = (int)((p->n + p->L - 1) / p->L);
+    {
+        auto gcd = [](long long a, long long b) { while (b) { const long long r = a % b; a = b; b = r; } return a; };
+        long long st = std::max<long long>(1, (long long)(0.6180339887 * p->ntiles));
+        while (gcd(st, p->ntiles) != 1) ++st;
+        p->tile_stride = (int)(st % p->ntiles == 0 ? 1 : st % p->ntiles);
+    }
     const bool per = o.dy_per_series != 0;
     p->M = per ? 3 * batch : batch + 2;
     const size_t B = real_bytes(dtype);

@@ -13,7 +13,7 @@
 
 namespace lsb {
 
-constexpr int kMaxWidth = 16;        // widest spreading kernel supported (cells)
+constexpr int kMaxWidth = 18;        // widest spreading kernel supported (cells)
 constexpr int kBinCells = 256;       // sort-bin length Lb in fine-grid cells (>= kMaxWidth/2 + 1)
 constexpr int kSpreadThreads = 256;  // threads per spreading CTA
 constexpr int kQuadNodes = 64;       // Gauss-Legendre nodes on [0,1] for psihat
@@ -54,6 +54,7 @@ struct ls_plan_s {
     int L = 1024;          // spreading tile length (cells), multiple of kBinCells
     int nbins = 0;         // ceil(n / kBinCells)
     int ntiles = 0;        // ceil(n / L)
+    int tile_stride = 1;   // launch-order permutation of the tiles: coprime to ntiles, ~0.618 ntiles
     int M = 0;             // transforms per execute
     int chunk = 1;         // series per pass
     int slots = 0;         // grid slots allocated

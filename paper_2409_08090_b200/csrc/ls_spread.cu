@@ -40,6 +40,7 @@ __device__ __forceinline__ float es_kernel(float z, float beta) {
 template <typename T>
 struct SpreadArgs {
     int n, L, nbins, w, H;          // H = ceil(w/2): candidate halo in cells
+    int ntiles, tile_stride;        // CTA b owns tile (b * tile_stride) mod ntiles (stride coprime to ntiles)
     T beta, two_over_w;
     const int* bin_start;
     const int* l0;
@@ -105,7 +106,9 @@ ls_spread_tile_kernel(const SpreadArgs<T> a) {
     int* start = cnt + HN;
     int* warp_tot = start + HN + 1;
 
-    const int tile = blockIdx.x;
+    // Occupied tiles (compute/latency-bound) and empty tiles (pure streaming stores) are interleaved in
+    // launch order by a multiplicative permutation, so the two kinds of work overlap on every SM.
+    const int tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
     const int row0 = blockIdx.y * NS;
     const int tile_lo = tile * a.L;
     const int Lt = min(a.L, a.n - tile_lo);
@@ -252,6 +255,8 @@ cudaError_t launch_t(ls_plan_s* p, int pointset, int row0, int nrows, int slot0,
     a.n = (int)p->n;
     a.L = p->L;
     a.nbins = p->nbins;
+    a.ntiles = p->ntiles;
+    a.tile_stride = p->tile_stride;
     a.w = p->w;
     a.H = (p->w + 1) / 2;
     a.beta = (T)p->beta;

@@ -38,7 +38,7 @@ def test_cfg1_full_grid():
     _check64(e)
     assert int(np.argmax(Pg[0])) == int(np.argmax(Po))
     assert ex["launches"][0] > 0 and ex["launches"][1] == 1            # our kernels ran; one cuFFT exec
-    assert ex["info"]["M"] == 3 and ex["info"]["n"] >= 2 * w.Nf - 2
+    assert ex["info"]["M"] == 3 and ex["info"]["n"] >= 1.25 * w.Nf
 
 
 def test_cfg2_full_grid_unsorted_times():
