@@ -83,6 +83,62 @@ void gauss_legendre_01(int Q, double* z, double* wt) {
     }
 }
 
+// Piecewise-polynomial fit of the ES kernel psi(s) = exp(beta (sqrt(1 - (2s/w)^2) - 1)) on each cell
+// of its support: Chebyshev interpolation in eta in [-1, 1] per piece, converted to
+// monomials in long double; the degree is raised until the measured error stops improving or is
+// below `tol`.  Only the first ceil(w/2) pieces are kept (psi is even).
+long double es_exact(long double s, int w, long double beta) {
+    const long double z = 2.0L * s / w;
+    const long double a = 1.0L - z * z;
+    return a > 0 ? expl(beta * (sqrtl(a) - 1.0L)) : expl(-beta);
+}
+
+void fit_kernel_poly(int w, double beta, double tol, lsb::KernelPoly* kp) {
+    const long double PI = 3.14159265358979323846264338327950288L;
+    const int half = (w + 1) / 2;
+    lsb::KernelPoly best{};
+    double prev_err = 1e300;
+    for (int D = 4; D <= lsb::kMaxDeg; D += 2) {
+        lsb::KernelPoly cur{};
+        cur.w = w; cur.deg = D; cur.half = half;
+        double worst = 0;
+        for (int i = 0; i < half; ++i) {
+            const long double centre = (long double)i - 0.5L * w + 0.5L;
+            long double f[lsb::kMaxDeg + 1], a[lsb::kMaxDeg + 1];
+            for (int j = 0; j <= D; ++j) f[j] = es_exact(cosl(PI * (j + 0.5L) / (D + 1)) / 2 + centre, w, beta);
+            for (int k = 0; k <= D; ++k) {
+                long double acc = 0;
+                for (int j = 0; j <= D; ++j) acc += f[j] * cosl(PI * k * (j + 0.5L) / (D + 1));
+                a[k] = acc * (k == 0 ? 1.0L : 2.0L) / (D + 1);
+            }
+            // sum_k a_k T_k(eta) -> monomials, T_{k+1} = 2 eta T_k - T_{k-1}
+            long double m[lsb::kMaxDeg + 1] = {0}, t0[lsb::kMaxDeg + 2] = {0}, t1[lsb::kMaxDeg + 2] = {0},
+                        t2[lsb::kMaxDeg + 2];
+            t0[0] = 1; t1[1] = 1;
+            m[0] += a[0];
+            if (D >= 1) m[1] += a[1];
+            for (int k = 2; k <= D; ++k) {
+                for (int d = 0; d <= D; ++d) t2[d] = (d > 0 ? 2 * t1[d - 1] : 0) - t0[d];
+                for (int d = 0; d <= D; ++d) { m[d] += a[k] * t2[d]; t0[d] = t1[d]; t1[d] = t2[d]; }
+            }
+            for (int d = 0; d <= lsb::kMaxDeg; ++d) cur.c[i][d] = d <= D ? (double)m[d] : 0.0;
+            for (int q = 0; q <= 64; ++q) {
+                const double eta = -1.0 + q / 32.0;
+                double v = 0;
+                for (int d = D; d >= 0; --d) v = v * eta + cur.c[i][d];
+                const double ex = (double)es_exact((long double)eta / 2 + centre, w, beta);
+                worst = std::max(worst, fabs(v - ex));
+            }
+        }
+        cur.max_err = worst;
+        if (worst > 0.5 * prev_err && best.deg) break;          // no longer improving: keep the previous degree
+        best = cur;
+        prev_err = worst;
+        if (worst <= tol) break;
+    }
+    *kp = best;
+}
+
 template <typename T>
 cudaError_t dmalloc(ls_plan_s* p, T** ptr, size_t bytes) {
     if (bytes == 0) bytes = 16;
@@ -172,15 +228,12 @@ int ls_destroy(ls_plan_t p) {
     cudaFree(p->fft_work);
     cudaFree(p->grids);
     cudaFree(p->dinv);
-    cudaFree(p->sums);
+    cudaFree(p->zeroed);                     // sums and both histograms live in this allocation
     cudaFree(p->scan_tmp);
-    cudaFree(p->ps[0].hist);                 // ps[1].hist points into the same allocation
     for (int i = 0; i < 2; ++i) {
         cudaFree(p->ps[i].bin_start);
-        cudaFree(p->ps[i].pos);
-        cudaFree(p->ps[i].l0);
-        cudaFree(p->ps[i].x0);
-        cudaFree(p->ps[i].q);
+        cudaFree(p->ps[i].perm);
+        cudaFree(p->ps[i].rec);
         cudaFree(p->ps[i].rows);
     }
     cudaFree(p->st_t);
@@ -250,7 +303,9 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     }
     p->w = w;
     p->beta = 0.97 * M_PI * w * (1.0 - 1.0 / (2.0 * std::min(p->sigma, 2.0)));
+    fit_kernel_poly(w, p->beta, 1e-3 * eps, &p->poly);
     p->L = o.tile_cells ? o.tile_cells : 1024;
+    if (batch > 1) p->L = std::min(p->L, 512);      // four transforms per CTA: two cells per thread
     p->nbins = (int)((p->n + lsb::kBinCells - 1) / lsb::kBinCells);
     p->ntiles = (int)((p->n + p->L - 1) / p->L);
     {
@@ -279,21 +334,22 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     do {
         if ((ce = dmalloc(p, &p->grids, (size_t)p->slots * grid_bytes)) != cudaSuccess) break;
         if ((ce = dmalloc(p, &p->dinv, (size_t)(Nf / 2 + 1) * 8)) != cudaSuccess) break;
-        if ((ce = dmalloc(p, &p->sums, (size_t)batch * 4 * 8)) != cudaSuccess) break;
+        // sums and both histograms live in ONE allocation so a single memset clears them per execute
+        const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
+        p->zeroed_bytes = sums_bytes + (size_t)2 * p->nbins * 4;
+        if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
+        p->sums = (double*)p->zeroed;
+        p->ps[0].hist = (int*)((char*)p->zeroed + sums_bytes);
+        p->ps[1].hist = p->ps[0].hist + p->nbins;
         const int nchunks = (p->nbins + 4095) / 4096;
         if ((ce = dmalloc(p, &p->scan_tmp, (size_t)2 * (nchunks + 1) * 4)) != cudaSuccess) break;
         if ((ce = cudaMemset(p->scan_tmp, 0, (size_t)2 * (nchunks + 1) * 4)) != cudaSuccess) break;
-        // both histograms live in ONE allocation so a single memset clears them
-        if ((ce = dmalloc(p, &p->ps[0].hist, (size_t)2 * p->nbins * 4)) != cudaSuccess) break;
-        p->ps[1].hist = p->ps[0].hist + p->nbins;
         for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
             lsb::PointSet& ps = p->ps[i];
             ps.nrows = i == 0 ? (per ? 2 * batch : batch + 1) : (per ? batch : 1);
             if ((ce = dmalloc(p, &ps.bin_start, (size_t)(p->nbins + 1) * 4)) != cudaSuccess) break;
-            if ((ce = dmalloc(p, &ps.pos, (size_t)Nd * 4)) != cudaSuccess) break;
-            if ((ce = dmalloc(p, &ps.l0, (size_t)Nd * 4)) != cudaSuccess) break;
-            if ((ce = dmalloc(p, (char**)&ps.x0, (size_t)Nd * B)) != cudaSuccess) break;
-            if ((ce = dmalloc(p, (char**)&ps.q, (size_t)Nd * 2 * B)) != cudaSuccess) break;
+            if (batch > 1 && (ce = dmalloc(p, &ps.perm, (size_t)Nd * 4)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, (char**)&ps.rec, (size_t)Nd * 4 * B)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&ps.rows, (size_t)ps.nrows * Nd * B)) != cudaSuccess) break;
         }
         if (ce != cudaSuccess) break;
@@ -365,20 +421,18 @@ int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* 
     const size_t total_slot = p->events_used;   // the TOTAL event pair is closed at the very end
     if (p->opts.timing) ++p->events_used;
 
-    stage_begin(p, LS_STAGE_STATS, s);
-    LS_TRY(cudaMemsetAsync(p->sums, 0, (size_t)p->batch * 4 * 8, s));
-    LS_TRY(lsb::launch_stats(p, (const double*)t, y, dy, s)); ++own;
+    stage_begin(p, LS_STAGE_STATS, s);              // K1 + the bin histogram of K3 (one kernel)
+    LS_TRY(cudaMemsetAsync(p->zeroed, 0, p->zeroed_bytes, s));
+    LS_TRY(lsb::launch_stats_count(p, (const double*)t, y, dy, s)); ++own;
     stage_end(p, s);
 
     stage_begin(p, LS_STAGE_SORT, s);
-    LS_TRY(cudaMemsetAsync(p->ps[0].hist, 0, (size_t)2 * p->nbins * 4, s));
-    LS_TRY(lsb::launch_bin_count(p, (const double*)t, s)); ++own;
     LS_TRY(lsb::launch_bin_scan(p, s)); own += 2;
     stage_end(p, s);
 
     stage_begin(p, LS_STAGE_PREMUL, s);
-    LS_TRY(lsb::launch_premultiply(p, (const double*)t, s)); ++own;
-    LS_TRY(lsb::launch_rows(p, y, dy, s)); ++own;
+    LS_TRY(lsb::launch_premultiply(p, (const double*)t, y, dy, s)); ++own;
+    if (p->batch > 1) { LS_TRY(lsb::launch_rows(p, y, dy, s)); ++own; }
     stage_end(p, s);
 
     {
@@ -389,17 +443,13 @@ int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* 
             stage_begin(p, LS_STAGE_SPREAD, s);
             if (per) {
                 // slots [0, C): w2_s ; slots [C, 3C): (w_s, h_s) pairs
-                LS_TRY(lsb::launch_spread(p, 1, ps.s0, ps.C, 0, s)); ++own;
-                LS_TRY(lsb::launch_spread(p, 0, 2 * ps.s0, 2 * ps.C, ps.C, s)); ++own;
+                LS_TRY(lsb::launch_spread(p, ps.s0, ps.C, 0, 2 * ps.s0, 2 * ps.C, ps.C, s)); ++own;
                 w2_slot = 0; w2_stride = 1; w_slot = ps.C; w_stride = 2; h_slot = ps.C + 1; h_stride = 2;
             } else {
                 // slot 0: w2, slot 1: w, slots 2..: h_s of this pass
-                if (ps.s0 == 0) {
-                    LS_TRY(lsb::launch_spread(p, 1, 0, 1, 0, s)); ++own;
-                    LS_TRY(lsb::launch_spread(p, 0, 0, 1 + ps.C, 1, s)); ++own;
-                } else {
-                    LS_TRY(lsb::launch_spread(p, 0, 1 + ps.s0, ps.C, 2, s)); ++own;
-                }
+                if (ps.s0 == 0) LS_TRY(lsb::launch_spread(p, 0, 1, 0, 0, 1 + ps.C, 1, s));
+                else LS_TRY(lsb::launch_spread(p, 0, 0, 0, 1 + ps.s0, ps.C, 2, s));
+                ++own;
                 w2_slot = 0; w2_stride = 0; w_slot = 1; w_stride = 0; h_slot = 2; h_stride = 1;
             }
             stage_end(p, s);

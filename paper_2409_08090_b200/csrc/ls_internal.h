@@ -14,23 +14,50 @@
 namespace lsb {
 
 constexpr int kMaxWidth = 18;        // widest spreading kernel supported (cells)
-constexpr int kBinCells = 256;       // sort-bin length Lb in fine-grid cells (>= kMaxWidth/2 + 1)
+constexpr int kBinCells = 64;        // sort-bin length in fine-grid cells (>= kMaxWidth/2 + 1)
 constexpr int kSpreadThreads = 256;  // threads per spreading CTA
+constexpr int kChunkPts = 256;       // candidates a spreading CTA stages per pass (one per thread)
 constexpr int kQuadNodes = 64;       // Gauss-Legendre nodes on [0,1] for psihat
+constexpr int kMaxDeg = 16;          // highest degree of the piecewise-polynomial kernel (even)
+constexpr int kHalfMax = (kMaxWidth + 1) / 2;
 
 // double-double constant (hi + lo), built on the host with FMA error-free products.
 struct dd {
     double hi, lo;
 };
 
+// Piecewise-polynomial form of the spreading kernel ("piecewise polynomial kernel
+// approximation"): on cell i of the support, psi(eta/2 + i - w/2 + 1/2) = sum_d c[i][d] eta^d for
+// eta in [-1, 1).  psi is even, so piece w-1-i is piece i at -eta: only ceil(w/2) pieces are kept
+// and each evaluation of (even part, odd part) yields two kernel values.
+struct KernelPoly {
+    int w = 0, deg = 0, half = 0;
+    double c[kHalfMax][kMaxDeg + 1];
+    double max_err = 0;              // measured on the host against exp/sqrt at plan time
+};
+
+// One bin-sorted non-uniform point, as the spreading kernel reads it (one 32-byte / 16-byte load).
+//   eta  position of the point inside its cell pattern: the first touched cell l0 lies
+//        x0 = (eta + 1)/2 - w/2 cells from the point, x0 in [-w/2, -w/2 + 1)
+//   l0   first fine-grid cell touched (unfolded: may be < 0 or >= n by less than w)
+//   q    unit phasor e^{2 pi i f_c t} (x1 point set) or its square (x2)
+struct __align__(32) Rec64 {
+    double eta;
+    int l0, pad;
+    double qx, qy;
+};
+struct __align__(16) Rec32 {
+    float eta;
+    int l0;
+    float qx, qy;
+};
+
 // One non-uniform point set in bin-sorted order (x1 = n df t, or x2 = 2 x1).
 struct PointSet {
     int* hist = nullptr;       // [nbins]   bin counts -> running cursors during the scatter
     int* bin_start = nullptr;  // [nbins+1] exclusive scan of the counts
-    int* pos = nullptr;        // [Nd]      sorted slot of input point j
-    int* l0 = nullptr;         // [Nd]      first fine-grid cell touched (unfolded, may be <0 or >=n)
-    void* x0 = nullptr;        // [Nd] T    offset of that cell from the point, in [-w/2, -w/2+1)
-    void* q = nullptr;         // [Nd] T2   unit phasor e^{2 pi i f_c t} (x1) or its square (x2)
+    int* perm = nullptr;       // [Nd]      input index of sorted slot s (batch > 1 only)
+    void* rec = nullptr;       // [Nd]      Rec64 / Rec32, sorted order
     void* rows = nullptr;      // [nrows][Nd] T  real strengths per transform, sorted order
     int nrows = 0;
 };
@@ -62,7 +89,10 @@ struct ls_plan_s {
     // device buffers
     void* grids = nullptr;      // [slots][n] complex T
     double* dinv = nullptr;     // [floor(Nf/2)+1] 1/psihat(k')
-    double* sums = nullptr;     // [batch][4]  (sum dy^-2, sum dy^-2 y, YY, unused)
+    double* sums = nullptr;     // [batch][4]  (sum dy^-2, sum dy^-2 y, YY, unused); first part of `zeroed`
+    void* zeroed = nullptr;     // sums + both histograms: one allocation, one memset per execute
+    size_t zeroed_bytes = 0;
+    lsb::KernelPoly poly;       // piecewise-polynomial spreading kernel (host copy; passed by value)
     int* scan_tmp = nullptr;    // block sums + ticket for the bin scan (both point sets)
     lsb::PointSet ps[2];
     // host staging for ls_execute_host
@@ -84,14 +114,17 @@ struct ls_plan_s {
 
 namespace lsb {
 
-// ---- ls_pre.cu: K1 stats, K3 bin count + scan, K2 premultiply + scatter --------------------
-cudaError_t launch_stats(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s);
-cudaError_t launch_bin_count(ls_plan_s* p, const double* t, cudaStream_t s);
+// ---- ls_pre.cu: K1 stats + K3 bin count, K3 scan, K2 premultiply + scatter (+ rows) -------
+cudaError_t launch_stats_count(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s);
 cudaError_t launch_bin_scan(ls_plan_s* p, cudaStream_t s);
-cudaError_t launch_premultiply(ls_plan_s* p, const double* t, cudaStream_t s);
+cudaError_t launch_premultiply(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s);
 cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_t s);
 // ---- ls_spread.cu: K4 ----------------------------------------------------------------------
-cudaError_t launch_spread(ls_plan_s* p, int pointset, int row0, int nrows, int slot0, cudaStream_t s);
+// One launch spreads rows [row0_x2, +nrows_x2) of the x2 point set into slots slot0_x2.. and rows
+// [row0_x1, +nrows_x1) of the x1 point set into slots slot0_x1.. (either count may be 0).
+cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int row0_x1, int nrows_x1,
+                          int slot0_x1, cudaStream_t s);
+int spread_rows_per_group(const ls_plan_s* p);
 // ---- ls_post.cu: P0 table, K5+K6 -----------------------------------------------------------
 cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double* weights, cudaStream_t s);
 cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,

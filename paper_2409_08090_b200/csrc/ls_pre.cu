@@ -16,8 +16,6 @@ namespace lsb {
 namespace {
 
 constexpr int kPreThreads = 256;
-constexpr int kPreItems = 4;                       // points per thread in the 1-D point kernels
-constexpr int kPreChunk = kPreThreads * kPreItems;
 constexpr int kScanThreads = 1024;
 constexpr int kScanItems = 4;
 constexpr int kScanChunk = kScanThreads * kScanItems;
@@ -75,45 +73,29 @@ __device__ __forceinline__ void support_start(double frac, int w, int& i0, doubl
     x0 = a - frac;
 }
 
-// ------------------------------------------------------------------------------ K1 stats
+// ------------------------------------------------------------------------------ K1 stats + K3 count
+// grid (point CTAs, batch), grid-stride over the points.  Every series accumulates sum dy^-2 y (and
+// sum dy^-2 when it has its own dy); the CTAs of series 0 also histogram the fine-grid bins of both
+// point sets.  One atomicAdd(double) per CTA and sum: the CTA count is capped by the launcher.
 template <typename T>
 __global__ void __launch_bounds__(kPreThreads)
-ls_stats_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __restrict__ sums,
-                long long Nd, int dy_per_series) {
+ls_stats_count_kernel(const double* __restrict__ t, const T* __restrict__ y, const T* __restrict__ dy,
+                      double* __restrict__ sums, long long Nd, int dy_per_series, dd ndf, int n,
+                      int* __restrict__ hist1, int* __restrict__ hist2) {
     __shared__ double red[kPreThreads / 32];
     const int s = blockIdx.y;
-    const long long base = (long long)blockIdx.x * kPreChunk;
     const T* ys = y + (long long)s * Nd;
     const T* ds = dy + (dy_per_series ? (long long)s * Nd : 0);
-    double a = 0.0, b = 0.0;
-#pragma unroll
-    for (int i = 0; i < kPreItems; ++i) {
-        const long long j = base + threadIdx.x + (long long)i * kPreThreads;
-        if (j < Nd) {
-            const double d = (double)ds[j];
-            const double iv = 1.0 / (d * d);
-            a += iv;
-            b += iv * (double)ys[j];
-        }
-    }
-    b = block_sum(b, red);
-    if (threadIdx.x == 0) atomicAdd(&sums[4 * s + 1], b);
-    if (dy_per_series || s == 0) {
-        a = block_sum(a, red);
-        if (threadIdx.x == 0) atomicAdd(&sums[4 * s + 0], a);
-    }
-}
-
-// ------------------------------------------------------------------------------ K3 bin count
-__global__ void __launch_bounds__(kPreThreads)
-ls_bin_count_kernel(const double* __restrict__ t, long long Nd, dd ndf, int n,
-                    int* __restrict__ hist1, int* __restrict__ hist2) {
-    const long long base = (long long)blockIdx.x * kPreChunk;
     const double dn = (double)n;
-#pragma unroll
-    for (int i = 0; i < kPreItems; ++i) {
-        const long long j = base + threadIdx.x + (long long)i * kPreThreads;
-        if (j < Nd) {
+    const bool need_w = dy_per_series || s == 0;
+    double a = 0.0, b = 0.0;
+    for (long long j = (long long)blockIdx.x * kPreThreads + threadIdx.x; j < Nd;
+         j += (long long)gridDim.x * kPreThreads) {
+        const double d = (double)ds[j];
+        const double iv = 1.0 / (d * d);
+        a += iv;
+        b += iv * (double)ys[j];
+        if (s == 0) {
             int c1, c2;
             double f1, f2;
             grid_coord(ndf, t[j], dn, c1, f1);
@@ -121,6 +103,12 @@ ls_bin_count_kernel(const double* __restrict__ t, long long Nd, dd ndf, int n,
             atomicAdd(&hist1[c1 / kBinCells], 1);
             atomicAdd(&hist2[c2 / kBinCells], 1);
         }
+    }
+    b = block_sum(b, red);
+    if (threadIdx.x == 0) atomicAdd(&sums[4 * s + 1], b);
+    if (need_w) {
+        a = block_sum(a, red);
+        if (threadIdx.x == 0) atomicAdd(&sums[4 * s + 0], a);
     }
 }
 
@@ -233,27 +221,48 @@ ls_bin_scan_apply_kernel(int* __restrict__ hist1, int* __restrict__ hist2, int* 
 
 // ------------------------------------------------------------------------------ K2 premultiply
 template <typename T>
-struct Cplx;
+struct RecOf;
 template <>
-struct Cplx<double> { using type = double2; };
+struct RecOf<double> { using type = Rec64; };
 template <>
-struct Cplx<float> { using type = float2; };
+struct RecOf<float> { using type = Rec32; };
 
-template <typename T>
+// One whole-record store: 32 bytes (STG.256) for fp64, 16 bytes for fp32.
+__device__ __forceinline__ void store_rec(Rec64* dst, double eta, int l0, double qx, double qy) {
+    const long long mid = (long long)(unsigned)l0;
+    asm volatile("st.global.v4.b64 [%0], {%1, %2, %3, %4};" ::"l"(dst), "l"(__double_as_longlong(eta)), "l"(mid),
+                 "l"(__double_as_longlong(qx)), "l"(__double_as_longlong(qy))
+                 : "memory");
+}
+__device__ __forceinline__ void store_rec(Rec32* dst, double eta, int l0, double qx, double qy) {
+    float4 v;
+    v.x = (float)eta;
+    v.y = __int_as_float(l0);
+    v.z = (float)qx;
+    v.w = (float)qy;
+    *reinterpret_cast<float4*>(dst) = v;
+}
+
+// grid-stride over the points.  FUSE_ROWS (batch == 1): the strengths w_j, h_j = w_j (y_j - ybar) of
+// the single series are scattered here too and YY is reduced, so no separate rows kernel runs.
+// Otherwise the sorted slot -> input index map `perm` is written for the gathering rows kernel.
+template <typename T, bool FUSE_ROWS>
 __global__ void __launch_bounds__(kPreThreads)
-ls_premultiply_kernel(const double* __restrict__ t, long long Nd, dd ndf, dd fc, int n, int w,
-                      int* __restrict__ cur1, int* __restrict__ cur2,
-                      int* __restrict__ pos1, int* __restrict__ pos2,
-                      int* __restrict__ l01, int* __restrict__ l02,
-                      T* __restrict__ x01, T* __restrict__ x02,
-                      typename Cplx<T>::type* __restrict__ q1, typename Cplx<T>::type* __restrict__ q2) {
-    using T2 = typename Cplx<T>::type;
-    const long long base = (long long)blockIdx.x * kPreChunk;
+ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, const T* __restrict__ dy,
+                      double* __restrict__ sums, long long Nd, dd ndf, dd fc, int n, int w,
+                      int* __restrict__ cur1, int* __restrict__ cur2, int* __restrict__ perm1,
+                      int* __restrict__ perm2, typename RecOf<T>::type* __restrict__ rec1,
+                      typename RecOf<T>::type* __restrict__ rec2, T* __restrict__ R1, T* __restrict__ R2) {
+    __shared__ double red[kPreThreads / 32];
     const double dn = (double)n;
-#pragma unroll
-    for (int i = 0; i < kPreItems; ++i) {
-        const long long j = base + threadIdx.x + (long long)i * kPreThreads;
-        if (j >= Nd) continue;
+    double W = 1.0, ybar = 0.0, yy = 0.0;
+    if (FUSE_ROWS) {
+        W = sums[0];
+        ybar = sums[1] / W;
+    }
+    const double invW = 1.0 / W;
+    for (long long j = (long long)blockIdx.x * kPreThreads + threadIdx.x; j < Nd;
+         j += (long long)gridDim.x * kPreThreads) {
         const double tj = t[j];
         int c1, c2, i1, i2;
         double f1, f2, xa, xb;
@@ -270,34 +279,40 @@ ls_premultiply_kernel(const double* __restrict__ t, long long Nd, dd ndf, dd fc,
         sincospi(2.0 * ph, &sn, &cs);
         const int s1 = atomicAdd(&cur1[c1 / kBinCells], 1);
         const int s2 = atomicAdd(&cur2[c2 / kBinCells], 1);
-        pos1[j] = s1;
-        pos2[j] = s2;
-        l01[s1] = c1 + i1;
-        l02[s2] = c2 + i2;
-        x01[s1] = (T)xa;
-        x02[s2] = (T)xb;
-        T2 a, b;
-        a.x = (T)cs;
-        a.y = (T)sn;
-        b.x = (T)(cs * cs - sn * sn);
-        b.y = (T)(2.0 * sn * cs);
-        q1[s1] = a;
-        q2[s2] = b;
+        // eta = 2 (x0 + w/2) - 1 in [-1, 1): argument of the piecewise-polynomial kernel
+        store_rec(&rec1[s1], 2.0 * xa + (double)(w - 1), c1 + i1, cs, sn);
+        store_rec(&rec2[s2], 2.0 * xb + (double)(w - 1), c2 + i2, cs * cs - sn * sn, 2.0 * sn * cs);
+        if (FUSE_ROWS) {
+            const double d = (double)dy[j];
+            const double wj = invW / (d * d);
+            const double yc = (double)y[j] - ybar;
+            R1[s1] = (T)wj;                     // row 0 of x1: w
+            R1[Nd + s1] = (T)(wj * yc);         // row 1 of x1: h
+            R2[s2] = (T)wj;                     // row 0 of x2: w
+            yy += wj * yc * yc;
+        } else {
+            perm1[s1] = (int)j;
+            perm2[s2] = (int)j;
+        }
+    }
+    if (FUSE_ROWS) {
+        yy = block_sum(yy, red);
+        if (threadIdx.x == 0) atomicAdd(&sums[2], yy);
     }
 }
 
 // ------------------------------------------------------------------------------ K2' rows + YY
-// grid (point chunks, batch).  Row layout:
+// batch > 1.  grid (slot CTAs, batch), grid-stride over SORTED slots: coalesced row writes, gathers
+// of y and dy through perm (one series is Nd reals: L1/L2-resident).  Row layout:
 //   shared dy:      R1 = [w ; h_0 .. h_{B-1}],  R2 = [w]
 //   per-series dy:  R1 = [w_0, h_0, w_1, h_1, ...],  R2 = [w_0, w_1, ...]
 template <typename T>
 __global__ void __launch_bounds__(kPreThreads)
 ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __restrict__ sums,
-               long long Nd, int dy_per_series, const int* __restrict__ pos1,
-               const int* __restrict__ pos2, T* __restrict__ R1, T* __restrict__ R2) {
+               long long Nd, int dy_per_series, const int* __restrict__ perm1,
+               const int* __restrict__ perm2, T* __restrict__ R1, T* __restrict__ R2) {
     __shared__ double red[kPreThreads / 32];
     const int s = blockIdx.y;
-    const long long base = (long long)blockIdx.x * kPreChunk;
     const T* ys = y + (long long)s * Nd;
     const T* ds = dy + (dy_per_series ? (long long)s * Nd : 0);
     const double W = sums[dy_per_series ? 4 * s : 0];
@@ -308,44 +323,44 @@ ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __rest
     T* roww2 = R2 + (long long)(dy_per_series ? s : 0) * Nd;
     const bool write_w = dy_per_series || s == 0;
     double yy = 0.0;
-#pragma unroll
-    for (int i = 0; i < kPreItems; ++i) {
-        const long long j = base + threadIdx.x + (long long)i * kPreThreads;
-        if (j < Nd) {
-            const double d = (double)ds[j];
-            const double wj = invW / (d * d);
-            const double yc = (double)ys[j] - ybar;
-            const int s1 = pos1[j];
-            rowh[s1] = (T)(wj * yc);
-            yy += wj * yc * yc;
-            if (write_w) {
-                roww1[s1] = (T)wj;
-                roww2[pos2[j]] = (T)wj;
-            }
+    for (long long q = (long long)blockIdx.x * kPreThreads + threadIdx.x; q < Nd;
+         q += (long long)gridDim.x * kPreThreads) {
+        const int j = perm1[q];
+        const double d = (double)ds[j];
+        const double wj = invW / (d * d);
+        const double yc = (double)ys[j] - ybar;
+        rowh[q] = (T)(wj * yc);
+        yy += wj * yc * yc;
+        if (write_w) {
+            roww1[q] = (T)wj;
+            const double d2 = (double)ds[perm2[q]];
+            roww2[q] = (T)(invW / (d2 * d2));
         }
     }
     yy = block_sum(yy, red);
     if (threadIdx.x == 0) atomicAdd(&sums[4 * s + 2], yy);
 }
 
-inline int point_blocks(long long Nd) { return (int)((Nd + kPreChunk - 1) / kPreChunk); }
+// CTAs along the points: enough to fill the machine, few enough that the one-per-CTA double atomics
+// on the per-series sums stay cheap.
+inline int point_blocks(long long Nd, int batch) {
+    const long long want = (Nd + kPreThreads - 1) / kPreThreads;
+    const long long cap = batch >= 64 ? 32 : 148 * 8;
+    return (int)(want < cap ? want : cap);
+}
 
 }  // namespace
 
-cudaError_t launch_stats(ls_plan_s* p, const double*, const void* y, const void* dy, cudaStream_t s) {
-    dim3 grid(point_blocks(p->Nd), p->batch);
+cudaError_t launch_stats_count(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s) {
+    dim3 grid(point_blocks(p->Nd, p->batch), p->batch);
     if (p->dtype == LS_F64)
-        ls_stats_kernel<double><<<grid, kPreThreads, 0, s>>>((const double*)y, (const double*)dy, p->sums, p->Nd,
-                                                             p->opts.dy_per_series);
+        ls_stats_count_kernel<double><<<grid, kPreThreads, 0, s>>>(t, (const double*)y, (const double*)dy, p->sums,
+                                                                   p->Nd, p->opts.dy_per_series, p->ndf, (int)p->n,
+                                                                   p->ps[0].hist, p->ps[1].hist);
     else
-        ls_stats_kernel<float><<<grid, kPreThreads, 0, s>>>((const float*)y, (const float*)dy, p->sums, p->Nd,
-                                                            p->opts.dy_per_series);
-    return cudaGetLastError();
-}
-
-cudaError_t launch_bin_count(ls_plan_s* p, const double* t, cudaStream_t s) {
-    ls_bin_count_kernel<<<point_blocks(p->Nd), kPreThreads, 0, s>>>(t, p->Nd, p->ndf, (int)p->n, p->ps[0].hist,
-                                                                    p->ps[1].hist);
+        ls_stats_count_kernel<float><<<grid, kPreThreads, 0, s>>>(t, (const float*)y, (const float*)dy, p->sums,
+                                                                  p->Nd, p->opts.dy_per_series, p->ndf, (int)p->n,
+                                                                  p->ps[0].hist, p->ps[1].hist);
     return cudaGetLastError();
 }
 
@@ -362,30 +377,36 @@ cudaError_t launch_bin_scan(ls_plan_s* p, cudaStream_t s) {
     return cudaGetLastError();
 }
 
-cudaError_t launch_premultiply(ls_plan_s* p, const double* t, cudaStream_t s) {
-    const int nb = point_blocks(p->Nd);
-    if (p->dtype == LS_F64)
-        ls_premultiply_kernel<double><<<nb, kPreThreads, 0, s>>>(
-            t, p->Nd, p->ndf, p->fc, (int)p->n, p->w, p->ps[0].hist, p->ps[1].hist, p->ps[0].pos, p->ps[1].pos,
-            p->ps[0].l0, p->ps[1].l0, (double*)p->ps[0].x0, (double*)p->ps[1].x0, (double2*)p->ps[0].q,
-            (double2*)p->ps[1].q);
+template <typename T>
+static cudaError_t premultiply_t(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s) {
+    using R = typename RecOf<T>::type;
+    const int nb = point_blocks(p->Nd, 1);
+    PointSet& a = p->ps[0];
+    PointSet& b = p->ps[1];
+    if (p->batch == 1)
+        ls_premultiply_kernel<T, true><<<nb, kPreThreads, 0, s>>>(
+            t, (const T*)y, (const T*)dy, p->sums, p->Nd, p->ndf, p->fc, (int)p->n, p->w, a.hist, b.hist, a.perm,
+            b.perm, (R*)a.rec, (R*)b.rec, (T*)a.rows, (T*)b.rows);
     else
-        ls_premultiply_kernel<float><<<nb, kPreThreads, 0, s>>>(
-            t, p->Nd, p->ndf, p->fc, (int)p->n, p->w, p->ps[0].hist, p->ps[1].hist, p->ps[0].pos, p->ps[1].pos,
-            p->ps[0].l0, p->ps[1].l0, (float*)p->ps[0].x0, (float*)p->ps[1].x0, (float2*)p->ps[0].q,
-            (float2*)p->ps[1].q);
+        ls_premultiply_kernel<T, false><<<nb, kPreThreads, 0, s>>>(
+            t, (const T*)y, (const T*)dy, p->sums, p->Nd, p->ndf, p->fc, (int)p->n, p->w, a.hist, b.hist, a.perm,
+            b.perm, (R*)a.rec, (R*)b.rec, (T*)a.rows, (T*)b.rows);
     return cudaGetLastError();
 }
 
+cudaError_t launch_premultiply(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s) {
+    return p->dtype == LS_F64 ? premultiply_t<double>(p, t, y, dy, s) : premultiply_t<float>(p, t, y, dy, s);
+}
+
 cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_t s) {
-    dim3 grid(point_blocks(p->Nd), p->batch);
+    dim3 grid(point_blocks(p->Nd, p->batch), p->batch);
     if (p->dtype == LS_F64)
         ls_rows_kernel<double><<<grid, kPreThreads, 0, s>>>((const double*)y, (const double*)dy, p->sums, p->Nd,
-                                                            p->opts.dy_per_series, p->ps[0].pos, p->ps[1].pos,
+                                                            p->opts.dy_per_series, p->ps[0].perm, p->ps[1].perm,
                                                             (double*)p->ps[0].rows, (double*)p->ps[1].rows);
     else
         ls_rows_kernel<float><<<grid, kPreThreads, 0, s>>>((const float*)y, (const float*)dy, p->sums, p->Nd,
-                                                           p->opts.dy_per_series, p->ps[0].pos, p->ps[1].pos,
+                                                           p->opts.dy_per_series, p->ps[0].perm, p->ps[1].perm,
                                                            (float*)p->ps[0].rows, (float*)p->ps[1].rows);
     return cudaGetLastError();
 }

@@ -1,25 +1,33 @@
 // ls_spread.cu — K4, tile-owner spreading ("upsample the data to
 // a fine grid"; spreading kernel = "exponential of semicircle" phi(z) = exp(beta (sqrt(1-z^2) - 1)),
-// PAPER.md:47, formula from the cited Barnett et al. 2019).
+// PAPER.md:47, formula from the cited Barnett et al. 2019, evaluated as a piecewise polynomial
+// ("piecewise polynomial kernel approximation") fitted at plan time).
 //
 //   b_l = sum_j c_j psi(l - u_j),  psi(s) = phi(2 s / w),  l taken mod n,
 //   c_j = q_j r_{m,j}: one unit phasor q_j per point, one REAL strength per (transform m, point).
 //
 // Design (differs from the paper's cuFINUFFT prior art): every CTA OWNS one tile of
 // L consecutive fine-grid cells of up to NS transforms and GATHERS the points whose support
-// overlaps it (its own sort bins plus one halo bin each side, periodic images included).  The
-// candidates are counting-sorted by first-touched cell in shared memory, then each thread
-// accumulates the cells it owns in REGISTERS and writes them once with coalesced 16-byte stores —
-// zeros included, so there is no memset pass, no global or shared floating-point atomic, and each
-// grid cell is written exactly once.  Tiles without points reduce to a pure streaming store.
+// overlaps it (its own sort bins plus one halo bin each side, periodic images included):
+//   1. each thread takes one candidate (one 32-byte record load), keys it by first-touched cell and
+//      ranks it with an integer shared-memory atomic;
+//   2. a block scan of the per-cell counts gives every candidate its slot in cell order;
+//   3. the candidate's thread evaluates its w kernel values by Horner (coefficients are warp-uniform
+//      kernel parameters; even/odd symmetry gives two values per evaluation) and stores them, with
+//      the NS complex strengths, at its slot;
+//   4. every thread then owns CPT consecutive cells, accumulates them in REGISTERS from the
+//      slot-ordered staging area and writes them once with 32-byte stores — zeros included.
+// There is no memset pass and no global or shared floating-point atomic; each grid cell is written
+// exactly once, and a tile without points is a pure streaming store.  One launch covers both point
+// sets (blockIdx.y) and the tiles are visited in a permuted order so that compute-bound occupied
+// tiles and store-bound empty tiles overlap on every SM.
 #include "ls_internal.h"
 
 namespace lsb {
 namespace {
 
-constexpr int kCellsPerThreadMax = 4;                 // L <= kSpreadThreads * 4
-constexpr int kChunkPts = 1024;                       // candidates staged per pass through smem
-constexpr int kPtsPerThread = kChunkPts / kSpreadThreads;
+constexpr int kScanPer = 5;                           // counts per thread in the block scan
+constexpr int kValStride = kChunkPts + 1;             // odd: conflict-free kernel-value staging
 
 template <typename T>
 struct V2;
@@ -27,38 +35,87 @@ template <>
 struct V2<double> { using type = double2; };
 template <>
 struct V2<float> { using type = float2; };
+template <typename T>
+struct RecOf;
+template <>
+struct RecOf<double> { using type = Rec64; };
+template <>
+struct RecOf<float> { using type = Rec32; };
 
-__device__ __forceinline__ double es_kernel(double z, double beta) {
-    const double a = fmax(0.0, 1.0 - z * z);
-    return exp(beta * (sqrt(a) - 1.0));
-}
-__device__ __forceinline__ float es_kernel(float z, float beta) {
-    const float a = fmaxf(0.0f, 1.0f - z * z);
-    return __expf(beta * (sqrtf(a) - 1.0f));
-}
+template <typename T>
+struct SpreadSeg {
+    const int* bin_start;
+    const typename RecOf<T>::type* rec;
+    const T* rows;                   // first row of this segment
+    typename V2<T>::type* grid;      // first slot of this segment, [nrows][n]
+    int nrows, ngroups;
+};
 
 template <typename T>
 struct SpreadArgs {
-    int n, L, nbins, w, H;          // H = ceil(w/2): candidate halo in cells
-    int ntiles, tile_stride;        // CTA b owns tile (b * tile_stride) mod ntiles (stride coprime to ntiles)
-    T beta, two_over_w;
-    const int* bin_start;
-    const int* l0;
-    const T* x0;
-    const typename V2<T>::type* q;
-    const T* rows;                   // first row of this launch
+    int n, L, nbins, w, H;           // H = ceil(w/2): candidate halo in cells
+    int ntiles, tile_stride;         // CTA b owns tile (b * tile_stride) mod ntiles
+    int deg, half;                   // polynomial degree (even), ceil(w/2) stored pieces
     long long Nd;
-    int nrows;
-    typename V2<T>::type* grid;      // first slot of this launch, [nrows][n]
+    SpreadSeg<T> seg[2];             // blockIdx.y < seg[0].ngroups: x2 rows, else x1 rows
+    T c[kHalfMax][kMaxDeg + 1];
 };
 
-// Block-wide exclusive scan of `cnt[0..len)` (len <= kSpreadThreads * 5) into `start[0..len]`.
-__device__ __forceinline__ void block_scan_counts(const int* cnt, int* start, int len, int* warp_tot) {
-    constexpr int PER = 5;
-    const int b = threadIdx.x * PER;
-    int v[PER], tsum = 0;
+__device__ __forceinline__ void load_rec(const Rec64* p, double& eta, int& l0, double& qx, double& qy) {
+    long long a, b, c, d;
+    asm volatile("ld.global.nc.v4.b64 {%0, %1, %2, %3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p));
+    eta = __longlong_as_double(a);
+    l0 = (int)(unsigned)(unsigned long long)b;
+    qx = __longlong_as_double(c);
+    qy = __longlong_as_double(d);
+}
+__device__ __forceinline__ void load_rec(const Rec32* p, float& eta, int& l0, float& qx, float& qy) {
+    const float4 v = __ldg(reinterpret_cast<const float4*>(p));
+    eta = v.x;
+    l0 = __float_as_int(v.y);
+    qx = v.z;
+    qy = v.w;
+}
+
+// CPT consecutive complex cells of one thread, written with the widest stores available.
+template <int CPT>
+__device__ __forceinline__ void store_cells(double2* dst, const double2 (&v)[CPT]) {
+    if constexpr (CPT % 2 == 0) {
 #pragma unroll
-    for (int i = 0; i < PER; ++i) {
+        for (int c = 0; c < CPT; c += 2)
+            asm volatile("st.global.v4.f64 [%0], {%1, %2, %3, %4};" ::"l"(dst + c), "d"(v[c].x), "d"(v[c].y),
+                         "d"(v[c + 1].x), "d"(v[c + 1].y)
+                         : "memory");
+    } else {
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) dst[c] = v[c];
+    }
+}
+template <int CPT>
+__device__ __forceinline__ void store_cells(float2* dst, const float2 (&v)[CPT]) {
+    if constexpr (CPT % 4 == 0) {
+#pragma unroll
+        for (int c = 0; c < CPT; c += 4)
+            asm volatile("st.global.v8.f32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"l"(dst + c), "f"(v[c].x),
+                         "f"(v[c].y), "f"(v[c + 1].x), "f"(v[c + 1].y), "f"(v[c + 2].x), "f"(v[c + 2].y),
+                         "f"(v[c + 3].x), "f"(v[c + 3].y)
+                         : "memory");
+    } else if constexpr (CPT % 2 == 0) {
+#pragma unroll
+        for (int c = 0; c < CPT; c += 2)
+            *reinterpret_cast<float4*>(dst + c) = make_float4(v[c].x, v[c].y, v[c + 1].x, v[c + 1].y);
+    } else {
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) dst[c] = v[c];
+    }
+}
+
+// Block-wide exclusive scan of cnt[0..len) (len <= kSpreadThreads * kScanPer) into start[0..len].
+__device__ __forceinline__ void block_scan_counts(const int* cnt, int* start, int len, int* warp_tot) {
+    const int b = threadIdx.x * kScanPer;
+    int v[kScanPer], tsum = 0;
+#pragma unroll
+    for (int i = 0; i < kScanPer; ++i) {
         v[i] = (b + i < len) ? cnt[b + i] : 0;
         tsum += v[i];
     }
@@ -72,7 +129,7 @@ __device__ __forceinline__ void block_scan_counts(const int* cnt, int* start, in
     if (lane == 31) warp_tot[wid] = inc;
     __syncthreads();
     if (wid == 0) {
-        int wv = (lane < kSpreadThreads / 32) ? warp_tot[lane] : 0;
+        const int wv = (lane < kSpreadThreads / 32) ? warp_tot[lane] : 0;
         int winc = wv;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -84,24 +141,24 @@ __device__ __forceinline__ void block_scan_counts(const int* cnt, int* start, in
     __syncthreads();
     int ex = warp_tot[wid] + inc - tsum;
 #pragma unroll
-    for (int i = 0; i < PER; ++i) {
+    for (int i = 0; i < kScanPer; ++i) {
         if (b + i <= len) start[b + i] = ex;
         ex += v[i];
     }
 }
 
-template <typename T, int NS>
-__global__ void __launch_bounds__(kSpreadThreads)
-ls_spread_tile_kernel(const SpreadArgs<T> a) {
+template <typename T, int NS, int CPT>
+__global__ void __launch_bounds__(kSpreadThreads, (NS * CPT <= 8) ? 4 : 3)
+ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     using T2 = typename V2<T>::type;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    // shared layout: q[kChunkPts] T2 | x0[kChunkPts] T | r[NS][kChunkPts] T | rel[kChunkPts] int |
+    // shared layout: sc[NS][kChunkPts] T2 | sval[w][kValStride] T | srel[kChunkPts] int |
     //                cnt[HN] int | start[HN+1] int | warp_tot[8] int
-    T2* sq = reinterpret_cast<T2*>(smem_raw);
-    T* sx = reinterpret_cast<T*>(sq + kChunkPts);
-    T* sr = sx + kChunkPts;
-    int* srel = reinterpret_cast<int*>(sr + NS * kChunkPts);
-    const int HN = a.L + a.w;                       // keys rel + (w-1) in [0, L + w - 1)
+    const int w = a.w;
+    T2* sc = reinterpret_cast<T2*>(smem_raw);
+    T* sval = reinterpret_cast<T*>(sc + NS * kChunkPts);
+    int* srel = reinterpret_cast<int*>(sval + w * kValStride);
+    const int HN = a.L + w;                         // keys rel + (w-1) in [0, L + w - 1)
     int* cnt = srel + kChunkPts;
     int* start = cnt + HN;
     int* warp_tot = start + HN + 1;
@@ -109,101 +166,119 @@ ls_spread_tile_kernel(const SpreadArgs<T> a) {
     // Occupied tiles (compute/latency-bound) and empty tiles (pure streaming stores) are interleaved in
     // launch order by a multiplicative permutation, so the two kinds of work overlap on every SM.
     const int tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
-    const int row0 = blockIdx.y * NS;
+    const int si = (int)blockIdx.y < a.seg[0].ngroups ? 0 : 1;
+    const SpreadSeg<T>& sg = a.seg[si];
+    const int row0 = ((int)blockIdx.y - (si ? a.seg[0].ngroups : 0)) * NS;
+    const int nr = min(NS, sg.nrows - row0);
     const int tile_lo = tile * a.L;
     const int Lt = min(a.L, a.n - tile_lo);
-    const int w = a.w;
 
     // Candidate pieces: cells [lo, hi) = [tile_lo - H, tile_lo + Lt + H); the parts below 0 / at or
     // above n are the periodic images (shift -n / +n applied to the point's cell).
     const int lo = tile_lo - a.H, hi = tile_lo + Lt + a.H;
     int pbeg[3], pcnt[3], pshift[3];
     {
-        // main piece
         const int mlo = max(lo, 0), mhi = min(hi, a.n);
-        pbeg[0] = a.bin_start[mlo / kBinCells];
-        pcnt[0] = a.bin_start[(mhi - 1) / kBinCells + 1] - pbeg[0];
+        pbeg[0] = __ldg(&sg.bin_start[mlo / kBinCells]);
+        pcnt[0] = __ldg(&sg.bin_start[(mhi - 1) / kBinCells + 1]) - pbeg[0];
         pshift[0] = 0;
-        // left image: cells [n + lo, n) shifted by -n
-        if (lo < 0) {
+        if (lo < 0) {                                // left image: cells [n + lo, n) shifted by -n
             const int c0 = max(a.n + lo, 0);
-            pbeg[1] = a.bin_start[c0 / kBinCells];
-            pcnt[1] = a.bin_start[a.nbins] - pbeg[1];
+            pbeg[1] = __ldg(&sg.bin_start[c0 / kBinCells]);
+            pcnt[1] = __ldg(&sg.bin_start[a.nbins]) - pbeg[1];
         } else { pbeg[1] = 0; pcnt[1] = 0; }
         pshift[1] = -a.n;
-        // right image: cells [0, hi - n) shifted by +n
-        if (hi > a.n) {
+        if (hi > a.n) {                              // right image: cells [0, hi - n) shifted by +n
             const int c1 = min(hi - a.n, a.n);
             pbeg[2] = 0;
-            pcnt[2] = a.bin_start[(c1 - 1) / kBinCells + 1];
+            pcnt[2] = __ldg(&sg.bin_start[(c1 - 1) / kBinCells + 1]);
         } else { pbeg[2] = 0; pcnt[2] = 0; }
         pshift[2] = a.n;
     }
     const int total = pcnt[0] + pcnt[1] + pcnt[2];
 
-    T2 acc[kCellsPerThreadMax][NS];
+    T2 acc[NS][CPT];
 #pragma unroll
-    for (int c = 0; c < kCellsPerThreadMax; ++c)
+    for (int s = 0; s < NS; ++s)
 #pragma unroll
-        for (int s = 0; s < NS; ++s) acc[c][s].x = acc[c][s].y = (T)0;
+        for (int c = 0; c < CPT; ++c) acc[s][c].x = acc[s][c].y = (T)0;
+
+    const int lbase = threadIdx.x * CPT;             // first owned cell, tile-relative
 
     for (int base = 0; base < total; base += kChunkPts) {
-        // ---- 1. count candidates of this chunk per first-touched cell
+        // ---- 1. one candidate per thread: record, key (first-touched cell), rank within its key
         for (int i = threadIdx.x; i < HN; i += kSpreadThreads) cnt[i] = 0;
         __syncthreads();
-        int g[kPtsPerThread], key[kPtsPerThread];
-#pragma unroll
-        for (int i = 0; i < kPtsPerThread; ++i) {
-            int ci = base + threadIdx.x + i * kSpreadThreads;
-            key[i] = -1;
-            g[i] = 0;
+        int key = -1, rank = 0, rel = 0;
+        T eta = (T)0, qx = (T)0, qy = (T)0, r[NS];
+        {
+            int ci = base + threadIdx.x;
             if (ci < total) {
-                int pc = 0;
-                if (ci >= pcnt[0]) { ci -= pcnt[0]; pc = 1; if (ci >= pcnt[1]) { ci -= pcnt[1]; pc = 2; } }
-                g[i] = pbeg[pc] + ci;
-                const int rel = a.l0[g[i]] + pshift[pc] - tile_lo;     // first touched cell, tile-relative
+                int g = pbeg[0] + ci, shift = 0;     // (selects, not indexed arrays: no local memory)
+                if (ci >= pcnt[0]) {
+                    ci -= pcnt[0];
+                    if (ci < pcnt[1]) { g = pbeg[1] + ci; shift = pshift[1]; }
+                    else { g = pbeg[2] + ci - pcnt[1]; shift = pshift[2]; }
+                }
+                int l0;
+                load_rec(sg.rec + g, eta, l0, qx, qy);
+                rel = l0 + shift - tile_lo;          // first touched cell, tile-relative
                 if (rel + w > 0 && rel < Lt) {
-                    key[i] = rel + w - 1;
-                    atomicAdd(&cnt[key[i]], 1);
+                    key = rel + w - 1;
+                    rank = atomicAdd(&cnt[key], 1);
+#pragma unroll
+                    for (int s = 0; s < NS; ++s)
+                        r[s] = (s < nr) ? __ldg(&sg.rows[(long long)(row0 + s) * a.Nd + g]) : (T)0;
                 }
             }
         }
         __syncthreads();
-        // ---- 2. exclusive scan -> start[]; cnt[] becomes the scatter cursor
+        // ---- 2. exclusive scan of the per-cell counts
         block_scan_counts(cnt, start, HN, warp_tot);
         __syncthreads();
-        for (int i = threadIdx.x; i < HN; i += kSpreadThreads) cnt[i] = start[i];
-        __syncthreads();
-        // ---- 3. scatter the candidates into cell order
+        // ---- 3. stage the candidate at its cell-ordered slot: strengths and w kernel values
+        if (key >= 0) {
+            const int slot = start[key] + rank;
+            srel[slot] = rel;
 #pragma unroll
-        for (int i = 0; i < kPtsPerThread; ++i) {
-            if (key[i] >= 0) {
-                const int slot = atomicAdd(&cnt[key[i]], 1);
-                sq[slot] = a.q[g[i]];
-                sx[slot] = a.x0[g[i]];
-                srel[slot] = key[i] - (w - 1);
-#pragma unroll
-                for (int s = 0; s < NS; ++s)
-                    sr[s * kChunkPts + slot] = (row0 + s < a.nrows) ? a.rows[(long long)(row0 + s) * a.Nd + g[i]] : (T)0;
+            for (int s = 0; s < NS; ++s) {
+                T2 cc;
+                cc.x = qx * r[s];
+                cc.y = qy * r[s];
+                sc[s * kChunkPts + slot] = cc;
+            }
+            const T z2 = eta * eta;
+            for (int i = 0; i < a.half; ++i) {
+                T e = (T)0, o = (T)0;
+                for (int d = a.deg; d >= 2; d -= 2) {
+                    e = fma(e, z2, a.c[i][d]);
+                    o = fma(o, z2, a.c[i][d - 1]);
+                }
+                e = fma(e, z2, a.c[i][0]);
+                o *= eta;
+                sval[i * kValStride + slot] = e + o;             // psi at cell l0 + i
+                sval[(w - 1 - i) * kValStride + slot] = e - o;   // psi at cell l0 + w-1-i (even symmetry)
             }
         }
         __syncthreads();
         // ---- 4. gather: cell l receives every point with rel in [l - w + 1, l], i.e. key in [l, l + w)
+        if (lbase < Lt) {
+            const int pe = start[lbase + CPT - 1 + w];
+            for (int pt = start[lbase]; pt < pe; ++pt) {
+                const int i0 = lbase - srel[pt];
+                T2 cs[NS];
 #pragma unroll
-        for (int c = 0; c < kCellsPerThreadMax; ++c) {
-            const int l = threadIdx.x + c * kSpreadThreads;
-            if (l < Lt) {
-                const int pe = start[l + w];
-                for (int pt = start[l]; pt < pe; ++pt) {
-                    const T z = (sx[pt] + (T)(l - srel[pt])) * a.two_over_w;
-                    const T k = es_kernel(z, a.beta);
-                    const T2 qq = sq[pt];
-                    const T kx = k * qq.x, ky = k * qq.y;
+                for (int s = 0; s < NS; ++s) cs[s] = sc[s * kChunkPts + pt];
 #pragma unroll
-                    for (int s = 0; s < NS; ++s) {
-                        const T r = sr[s * kChunkPts + pt];
-                        acc[c][s].x = fma(kx, r, acc[c][s].x);
-                        acc[c][s].y = fma(ky, r, acc[c][s].y);
+                for (int c = 0; c < CPT; ++c) {
+                    const int i = i0 + c;
+                    if ((unsigned)i < (unsigned)w) {
+                        const T k = sval[i * kValStride + pt];
+#pragma unroll
+                        for (int s = 0; s < NS; ++s) {
+                            acc[s][c].x = fma(k, cs[s].x, acc[s][c].x);
+                            acc[s][c].y = fma(k, cs[s].y, acc[s][c].y);
+                        }
                     }
                 }
             }
@@ -212,14 +287,18 @@ ls_spread_tile_kernel(const SpreadArgs<T> a) {
     }
 
     // ---- 5. the tile is written exactly once (zeros included)
+    if (lbase < Lt) {
 #pragma unroll
-    for (int s = 0; s < NS; ++s) {
-        if (row0 + s < a.nrows) {
-            T2* out = a.grid + (long long)(row0 + s) * a.n + tile_lo;
+        for (int s = 0; s < NS; ++s) {
+            if (s < nr) {
+                T2* out = sg.grid + (long long)(row0 + s) * a.n + tile_lo + lbase;
+                if (lbase + CPT <= Lt) {
+                    store_cells<CPT>(out, acc[s]);
+                } else {
 #pragma unroll
-            for (int c = 0; c < kCellsPerThreadMax; ++c) {
-                const int l = threadIdx.x + c * kSpreadThreads;
-                if (l < Lt) out[l] = acc[c][s];
+                    for (int c = 0; c < CPT; ++c)
+                        if (lbase + c < Lt) out[c] = acc[s][c];
+                }
             }
         }
     }
@@ -228,58 +307,74 @@ ls_spread_tile_kernel(const SpreadArgs<T> a) {
 template <typename T, int NS>
 size_t spread_smem_bytes(int L, int w) {
     const int HN = L + w;
-    return sizeof(typename V2<T>::type) * kChunkPts + sizeof(T) * kChunkPts * (1 + NS) + sizeof(int) * kChunkPts +
+    return sizeof(typename V2<T>::type) * NS * kChunkPts + sizeof(T) * (size_t)w * kValStride + sizeof(int) * kChunkPts +
            sizeof(int) * (HN + HN + 1 + 8);
 }
 
-template <typename T, int NS>
-cudaError_t launch_ns(ls_plan_s* p, const SpreadArgs<T>& a, cudaStream_t s) {
-    static bool configured = false;
-    const size_t smem = spread_smem_bytes<T, NS>(p->L, p->w);
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(ls_spread_tile_kernel<T, NS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)spread_smem_bytes<T, NS>(kSpreadThreads * kCellsPerThreadMax, kMaxWidth));
+template <typename T, int NS, int CPT>
+cudaError_t launch_inst(ls_plan_s* p, const SpreadArgs<T>& a, cudaStream_t s) {
+    static bool configured[64] = {false};          // per device: the attribute belongs to the device's function
+    const int dev = p->opts.device & 63;
+    if (!configured[dev]) {
+        cudaError_t e = cudaFuncSetAttribute(ls_spread_tile_kernel<T, NS, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)spread_smem_bytes<T, NS>(kSpreadThreads * CPT, kMaxWidth));
         if (e != cudaSuccess) return e;
-        configured = true;
+        configured[dev] = true;
     }
-    dim3 grid(p->ntiles, (a.nrows + NS - 1) / NS);
-    ls_spread_tile_kernel<T, NS><<<grid, kSpreadThreads, smem, s>>>(a);
+    dim3 grid(p->ntiles, a.seg[0].ngroups + a.seg[1].ngroups);
+    ls_spread_tile_kernel<T, NS, CPT><<<grid, kSpreadThreads, spread_smem_bytes<T, NS>(p->L, p->w), s>>>(a);
     return cudaGetLastError();
 }
 
 template <typename T>
-cudaError_t launch_t(ls_plan_s* p, int pointset, int row0, int nrows, int slot0, cudaStream_t s) {
+cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int row0_x1, int nrows_x1, int slot0_x1,
+                     cudaStream_t s) {
     using T2 = typename V2<T>::type;
-    const PointSet& ps = p->ps[pointset];
+    using R = typename RecOf<T>::type;
+    const int NS = spread_rows_per_group(p);
     SpreadArgs<T> a;
     a.n = (int)p->n;
     a.L = p->L;
     a.nbins = p->nbins;
-    a.ntiles = p->ntiles;
-    a.tile_stride = p->tile_stride;
     a.w = p->w;
     a.H = (p->w + 1) / 2;
-    a.beta = (T)p->beta;
-    a.two_over_w = (T)(2.0 / p->w);
-    a.bin_start = ps.bin_start;
-    a.l0 = ps.l0;
-    a.x0 = (const T*)ps.x0;
-    a.q = (const T2*)ps.q;
-    a.rows = (const T*)ps.rows + (long long)row0 * p->Nd;
+    a.ntiles = p->ntiles;
+    a.tile_stride = p->tile_stride;
+    a.deg = p->poly.deg;
+    a.half = p->poly.half;
     a.Nd = p->Nd;
-    a.nrows = nrows;
-    a.grid = (T2*)p->grids + (long long)slot0 * p->n;
-    if (nrows == 1) return launch_ns<T, 1>(p, a, s);
-    if (nrows == 2) return launch_ns<T, 2>(p, a, s);
-    return launch_ns<T, 4>(p, a, s);
+    for (int i = 0; i < kHalfMax; ++i)
+        for (int d = 0; d <= kMaxDeg; ++d) a.c[i][d] = (T)p->poly.c[i][d];
+    const int row0[2] = {row0_x2, row0_x1}, nrows[2] = {nrows_x2, nrows_x1}, slot0[2] = {slot0_x2, slot0_x1};
+    for (int g = 0; g < 2; ++g) {
+        const PointSet& ps = p->ps[g == 0 ? 1 : 0];
+        a.seg[g].bin_start = ps.bin_start;
+        a.seg[g].rec = (const R*)ps.rec;
+        a.seg[g].rows = (const T*)ps.rows + (long long)row0[g] * p->Nd;
+        a.seg[g].grid = (T2*)p->grids + (long long)slot0[g] * p->n;
+        a.seg[g].nrows = nrows[g];
+        a.seg[g].ngroups = (nrows[g] + NS - 1) / NS;
+    }
+    const int cpt = p->L / kSpreadThreads;
+    if (NS == 2) {
+        if (cpt == 4) return launch_inst<T, 2, 4>(p, a, s);
+        if (cpt == 2) return launch_inst<T, 2, 2>(p, a, s);
+        return launch_inst<T, 2, 1>(p, a, s);
+    }
+    if (cpt == 2) return launch_inst<T, 4, 2>(p, a, s);
+    return launch_inst<T, 4, 1>(p, a, s);
 }
 
 }  // namespace
 
-cudaError_t launch_spread(ls_plan_s* p, int pointset, int row0, int nrows, int slot0, cudaStream_t s) {
-    if (nrows <= 0) return cudaSuccess;
-    return p->dtype == LS_F64 ? launch_t<double>(p, pointset, row0, nrows, slot0, s)
-                              : launch_t<float>(p, pointset, row0, nrows, slot0, s);
+// Transforms accumulated per CTA: 2 for a single series ({w, h} at x1), 4 for a batch.
+int spread_rows_per_group(const ls_plan_s* p) { return p->batch == 1 ? 2 : 4; }
+
+cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int row0_x1, int nrows_x1,
+                          int slot0_x1, cudaStream_t s) {
+    if (nrows_x2 <= 0 && nrows_x1 <= 0) return cudaSuccess;
+    return p->dtype == LS_F64 ? launch_t<double>(p, row0_x2, nrows_x2, slot0_x2, row0_x1, nrows_x1, slot0_x1, s)
+                              : launch_t<float>(p, row0_x2, nrows_x2, slot0_x2, row0_x1, nrows_x1, slot0_x1, s);
 }
 
 }  // namespace lsb
