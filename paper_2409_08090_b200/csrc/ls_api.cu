@@ -93,12 +93,12 @@ long double es_exact(long double s, int w, long double beta) {
     return a > 0 ? expl(beta * (sqrtl(a) - 1.0L)) : expl(-beta);
 }
 
-void fit_kernel_poly(int w, double beta, double tol, lsb::KernelPoly* kp) {
+void fit_kernel_poly(int w, double beta, double tol, int max_deg, lsb::KernelPoly* kp) {
     const long double PI = 3.14159265358979323846264338327950288L;
     const int half = (w + 1) / 2;
     lsb::KernelPoly best{};
     double prev_err = 1e300;
-    for (int D = 4; D <= lsb::kMaxDeg; D += 2) {
+    for (int D = 4; D <= max_deg; D += 2) {
         lsb::KernelPoly cur{};
         cur.w = w; cur.deg = D; cur.half = half;
         double worst = 0;
@@ -303,7 +303,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     }
     p->w = w;
     p->beta = 0.97 * M_PI * w * (1.0 - 1.0 / (2.0 * std::min(p->sigma, 2.0)));
-    fit_kernel_poly(w, p->beta, 1e-3 * eps, &p->poly);
+    fit_kernel_poly(w, p->beta, 1e-3 * eps, dtype == LS_F64 ? 12 : 8, &p->poly);
     p->L = o.tile_cells ? o.tile_cells : 1024;
     if (batch > 1) p->L = std::min(p->L, 512);      // four transforms per CTA: two cells per thread
     p->nbins = (int)((p->n + lsb::kBinCells - 1) / lsb::kBinCells);

@@ -18,7 +18,7 @@ constexpr int kBinCells = 64;        // sort-bin length in fine-grid cells (>= k
 constexpr int kSpreadThreads = 256;  // threads per spreading CTA
 constexpr int kChunkPts = 256;       // candidates a spreading CTA stages per pass (one per thread)
 constexpr int kQuadNodes = 64;       // Gauss-Legendre nodes on [0,1] for psihat
-constexpr int kMaxDeg = 16;          // highest degree of the piecewise-polynomial kernel (even)
+constexpr int kMaxDeg = 12;          // highest degree of the piecewise-polynomial kernel (even; fp32 uses 8)
 constexpr int kHalfMax = (kMaxWidth + 1) / 2;
 
 // double-double constant (hi + lo), built on the host with FMA error-free products.

@@ -55,10 +55,11 @@ template <typename T>
 struct SpreadArgs {
     int n, L, nbins, w, H;           // H = ceil(w/2): candidate halo in cells
     int ntiles, tile_stride;         // CTA b owns tile (b * tile_stride) mod ntiles
-    int deg, half;                   // polynomial degree (even), ceil(w/2) stored pieces
+    int tile_mask;                   // ntiles - 1 when ntiles is a power of two, else -1
+    int half;                        // ceil(w/2) stored polynomial pieces
     long long Nd;
     SpreadSeg<T> seg[2];             // blockIdx.y < seg[0].ngroups: x2 rows, else x1 rows
-    T c[kHalfMax][kMaxDeg + 1];
+    T c[kHalfMax][kMaxDeg + 1];      // only degrees <= PolyDeg<T> are read
 };
 
 __device__ __forceinline__ void load_rec(const Rec64* p, double& eta, int& l0, double& qx, double& qy) {
@@ -110,13 +111,18 @@ __device__ __forceinline__ void store_cells(float2* dst, const float2 (&v)[CPT])
     }
 }
 
-// Block-wide exclusive scan of cnt[0..len) (len <= kSpreadThreads * kScanPer) into start[0..len].
-__device__ __forceinline__ void block_scan_counts(const int* cnt, int* start, int len, int* warp_tot) {
+// Block-wide exclusive scan of cnt[0..len) (len <= kSpreadThreads * kScanPer) into start[0..len];
+// cnt is left zeroed.
+__device__ __forceinline__ void block_scan_counts(int* cnt, int* start, int len, int* warp_tot) {
     const int b = threadIdx.x * kScanPer;
     int v[kScanPer], tsum = 0;
 #pragma unroll
     for (int i = 0; i < kScanPer; ++i) {
-        v[i] = (b + i < len) ? cnt[b + i] : 0;
+        v[i] = 0;
+        if (b + i < len) {
+            v[i] = cnt[b + i];
+            cnt[b + i] = 0;                          // ready for the next chunk of candidates
+        }
         tsum += v[i];
     }
     const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
@@ -147,10 +153,21 @@ __device__ __forceinline__ void block_scan_counts(const int* cnt, int* start, in
     }
 }
 
+// Polynomial degree the kernels unroll to (coefficients above the fitted degree are zero):
+// 12 reaches the sqrt-singularity floor of the ES kernel (<= 7e-13) for every fp64 width, 8 is
+// below 1e-7 for every fp32 width (measured at plan time, KernelPoly::max_err).
+template <typename T>
+struct PolyDeg;
+template <>
+struct PolyDeg<double> { static constexpr int value = 12; };
+template <>
+struct PolyDeg<float> { static constexpr int value = 8; };
+
 template <typename T, int NS, int CPT>
 __global__ void __launch_bounds__(kSpreadThreads, (NS * CPT <= 8) ? 4 : 3)
 ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     using T2 = typename V2<T>::type;
+    constexpr int DEG = PolyDeg<T>::value;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     // shared layout: sc[NS][kChunkPts] T2 | sval[w][kValStride] T | srel[kChunkPts] int |
     //                cnt[HN] int | start[HN+1] int | warp_tot[8] int
@@ -165,7 +182,10 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
 
     // Occupied tiles (compute/latency-bound) and empty tiles (pure streaming stores) are interleaved in
     // launch order by a multiplicative permutation, so the two kinds of work overlap on every SM.
-    const int tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
+    int tile;
+    if (a.tile_mask >= 0) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) & (unsigned)a.tile_mask);
+    else if (a.ntiles <= 65535) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) % (unsigned)a.ntiles);
+    else tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
     const int si = (int)blockIdx.y < a.seg[0].ngroups ? 0 : 1;
     const SpreadSeg<T>& sg = a.seg[si];
     const int row0 = ((int)blockIdx.y - (si ? a.seg[0].ngroups : 0)) * NS;
@@ -176,26 +196,19 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     // Candidate pieces: cells [lo, hi) = [tile_lo - H, tile_lo + Lt + H); the parts below 0 / at or
     // above n are the periodic images (shift -n / +n applied to the point's cell).
     const int lo = tile_lo - a.H, hi = tile_lo + Lt + a.H;
-    int pbeg[3], pcnt[3], pshift[3];
+    int pbeg0, pcnt0, pbeg1 = 0, pcnt1 = 0, pcnt2 = 0;
     {
         const int mlo = max(lo, 0), mhi = min(hi, a.n);
-        pbeg[0] = __ldg(&sg.bin_start[mlo / kBinCells]);
-        pcnt[0] = __ldg(&sg.bin_start[(mhi - 1) / kBinCells + 1]) - pbeg[0];
-        pshift[0] = 0;
+        pbeg0 = __ldg(&sg.bin_start[mlo / kBinCells]);
+        pcnt0 = __ldg(&sg.bin_start[(mhi - 1) / kBinCells + 1]) - pbeg0;
         if (lo < 0) {                                // left image: cells [n + lo, n) shifted by -n
-            const int c0 = max(a.n + lo, 0);
-            pbeg[1] = __ldg(&sg.bin_start[c0 / kBinCells]);
-            pcnt[1] = __ldg(&sg.bin_start[a.nbins]) - pbeg[1];
-        } else { pbeg[1] = 0; pcnt[1] = 0; }
-        pshift[1] = -a.n;
-        if (hi > a.n) {                              // right image: cells [0, hi - n) shifted by +n
-            const int c1 = min(hi - a.n, a.n);
-            pbeg[2] = 0;
-            pcnt[2] = __ldg(&sg.bin_start[(c1 - 1) / kBinCells + 1]);
-        } else { pbeg[2] = 0; pcnt[2] = 0; }
-        pshift[2] = a.n;
+            pbeg1 = __ldg(&sg.bin_start[max(a.n + lo, 0) / kBinCells]);
+            pcnt1 = __ldg(&sg.bin_start[a.nbins]) - pbeg1;
+        }
+        if (hi > a.n)                                // right image: cells [0, hi - n) shifted by +n
+            pcnt2 = __ldg(&sg.bin_start[(min(hi - a.n, a.n) - 1) / kBinCells + 1]);
     }
-    const int total = pcnt[0] + pcnt[1] + pcnt[2];
+    const int total = pcnt0 + pcnt1 + pcnt2;
 
     T2 acc[NS][CPT];
 #pragma unroll
@@ -206,38 +219,46 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     const int lbase = threadIdx.x * CPT;             // first owned cell, tile-relative
 
     for (int base = 0; base < total; base += kChunkPts) {
-        // ---- 1. one candidate per thread: record, key (first-touched cell), rank within its key
-        for (int i = threadIdx.x; i < HN; i += kSpreadThreads) cnt[i] = 0;
-        __syncthreads();
-        int key = -1, rank = 0, rel = 0;
+        // ---- 1. one candidate per thread: its record and strengths (loads issued before the barrier)
+        bool have = false;
+        int rel = 0;
         T eta = (T)0, qx = (T)0, qy = (T)0, r[NS];
+#pragma unroll
+        for (int s = 0; s < NS; ++s) r[s] = (T)0;
         {
             int ci = base + threadIdx.x;
             if (ci < total) {
-                int g = pbeg[0] + ci, shift = 0;     // (selects, not indexed arrays: no local memory)
-                if (ci >= pcnt[0]) {
-                    ci -= pcnt[0];
-                    if (ci < pcnt[1]) { g = pbeg[1] + ci; shift = pshift[1]; }
-                    else { g = pbeg[2] + ci - pcnt[1]; shift = pshift[2]; }
+                int g = pbeg0 + ci, shift = 0;
+                if (ci >= pcnt0) {
+                    ci -= pcnt0;
+                    if (ci < pcnt1) { g = pbeg1 + ci; shift = -a.n; }
+                    else { g = ci - pcnt1; shift = a.n; }
                 }
                 int l0;
                 load_rec(sg.rec + g, eta, l0, qx, qy);
                 rel = l0 + shift - tile_lo;          // first touched cell, tile-relative
-                if (rel + w > 0 && rel < Lt) {
-                    key = rel + w - 1;
-                    rank = atomicAdd(&cnt[key], 1);
+                have = rel + w > 0 && rel < Lt;
+                if (have) {
 #pragma unroll
                     for (int s = 0; s < NS; ++s)
-                        r[s] = (s < nr) ? __ldg(&sg.rows[(long long)(row0 + s) * a.Nd + g]) : (T)0;
+                        if (s < nr) r[s] = __ldg(&sg.rows[(long long)(row0 + s) * a.Nd + g]);
                 }
             }
         }
+        if (base == 0) {                             // later chunks find cnt re-zeroed by the scan
+            for (int i = threadIdx.x; i < HN; i += kSpreadThreads) cnt[i] = 0;
+            __syncthreads();
+        }
+        // key = first-touched cell + (w - 1); rank = arrival order among equal keys
+        const int key = rel + w - 1;
+        int rank = 0;
+        if (have) rank = atomicAdd(&cnt[key], 1);
         __syncthreads();
-        // ---- 2. exclusive scan of the per-cell counts
+        // ---- 2. exclusive scan of the per-cell counts (re-zeroes cnt for the next chunk)
         block_scan_counts(cnt, start, HN, warp_tot);
         __syncthreads();
         // ---- 3. stage the candidate at its cell-ordered slot: strengths and w kernel values
-        if (key >= 0) {
+        if (have) {
             const int slot = start[key] + rank;
             srel[slot] = rel;
 #pragma unroll
@@ -248,16 +269,20 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
                 sc[s * kChunkPts + slot] = cc;
             }
             const T z2 = eta * eta;
-            for (int i = 0; i < a.half; ++i) {
-                T e = (T)0, o = (T)0;
-                for (int d = a.deg; d >= 2; d -= 2) {
-                    e = fma(e, z2, a.c[i][d]);
-                    o = fma(o, z2, a.c[i][d - 1]);
+#pragma unroll
+            for (int i = 0; i < kHalfMax; ++i) {
+                if (i < a.half) {                    // warp-uniform; coefficients are constant-bank operands
+                    T e = a.c[i][DEG], o = a.c[i][DEG - 1];
+#pragma unroll
+                    for (int d = DEG - 2; d >= 2; d -= 2) {
+                        e = fma(e, z2, a.c[i][d]);
+                        o = fma(o, z2, a.c[i][d - 1]);
+                    }
+                    e = fma(e, z2, a.c[i][0]);
+                    o *= eta;
+                    sval[i * kValStride + slot] = e + o;             // psi at cell l0 + i
+                    sval[(w - 1 - i) * kValStride + slot] = e - o;   // psi at cell l0 + w-1-i (even symmetry)
                 }
-                e = fma(e, z2, a.c[i][0]);
-                o *= eta;
-                sval[i * kValStride + slot] = e + o;             // psi at cell l0 + i
-                sval[(w - 1 - i) * kValStride + slot] = e - o;   // psi at cell l0 + w-1-i (even symmetry)
             }
         }
         __syncthreads();
@@ -283,7 +308,7 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
                 }
             }
         }
-        __syncthreads();
+        if (base + kChunkPts < total) __syncthreads();   // staging area is reused by the next chunk
     }
 
     // ---- 5. the tile is written exactly once (zeros included)
@@ -340,7 +365,7 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.H = (p->w + 1) / 2;
     a.ntiles = p->ntiles;
     a.tile_stride = p->tile_stride;
-    a.deg = p->poly.deg;
+    a.tile_mask = (p->ntiles & (p->ntiles - 1)) == 0 ? p->ntiles - 1 : -1;
     a.half = p->poly.half;
     a.Nd = p->Nd;
     for (int i = 0; i < kHalfMax; ++i)
