@@ -49,6 +49,11 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--cpu-freqs", type=int, default=0, help="oracle sample size (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (tuning runs)")
+    # plan tuning knobs (ls_opts); 0 = the library's automatic choice
+    ap.add_argument("--tile-cells", type=int, default=0)
+    ap.add_argument("--upsampfac", type=float, default=0.0)
+    ap.add_argument("--kernel-width", type=int, default=0)
     return ap.parse_args()
 
 
@@ -221,7 +226,8 @@ def run_ours(args):
     hP = torch.empty((w.batch, w.Nf), dtype=tdt).pin_memory()
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     plan = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F64 if w.dtype == "f64" else B.LS_F32, w.batch,
-                  timing=1, device=local)
+                  timing=1, device=local, tile_cells=args.tile_cells, upsampfac=args.upsampfac,
+                  kernel_width=args.kernel_width)
     info = plan.info
     stream = torch.cuda.current_stream().cuda_stream
 
@@ -257,11 +263,11 @@ def run_ours(args):
     dev_ms = float(np.sum(step_ms))
 
     # ---- e2e leg: host buffers through ls_execute_host (H2D + D2H inside the timed region)
-    for _ in range(2):
+    for _ in range(0 if args.no_e2e else 2):
         plan.execute_host(ht, hy, hdy, hP, stream)
     e2e_ms = 0.0
     barrier()
-    for i in range(args.steps):
+    for i in range(0 if args.no_e2e else args.steps):
         flush.fill_(i & 0xFF)
         torch.cuda.synchronize()
         t0 = time.perf_counter()

@@ -40,10 +40,11 @@ inline dd dd_add_d(dd a, double b) {
     return r;
 }
 
-// smallest even integer >= lo whose prime factors are all in {2, 3, 5}
+// smallest multiple of 4 >= lo whose prime factors are all in {2, 3, 5} (a multiple of 4 keeps every
+// grid row 32-byte aligned for the vector stores of the spreading kernel, fp32 included)
 int64_t next_smooth_even(int64_t lo) {
-    if (lo < 2) lo = 2;
-    for (int64_t m = lo + (lo & 1);; m += 2) {
+    if (lo < 4) lo = 4;
+    for (int64_t m = (lo + 3) / 4 * 4;; m += 4) {
         int64_t r = m;
         while (r % 2 == 0) r /= 2;
         while (r % 3 == 0) r /= 3;
@@ -276,6 +277,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (!p) return LS_ERR_ALLOC;
     p->Nd = Nd; p->Nf = Nf; p->f0 = f0; p->df = df; p->eps = eps; p->dtype = dtype; p->batch = batch;
     p->opts = o;
+    if (cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, o.device) != cudaSuccess || p->num_sms < 1) {
+        cudaGetLastError();
+        p->num_sms = 148;
+    }
 
     // ---- (sigma, w, beta, n) from eps: reading A10.  Auto: the fine grid is the power of two in
     // [1.25 Nf, 2.5 Nf) (the FFT pass count, not the cell count, decides its time), the

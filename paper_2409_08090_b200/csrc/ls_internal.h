@@ -81,6 +81,7 @@ struct ls_plan_s {
     int L = 1024;          // spreading tile length (cells), multiple of kBinCells
     int nbins = 0;         // ceil(n / kBinCells)
     int ntiles = 0;        // ceil(n / L)
+    int num_sms = 148;     // multiprocessors of the plan's device (filler CTAs of the spread kernel)
     int tile_stride = 1;   // launch-order permutation of the tiles: coprime to ntiles, ~0.618 ntiles
     int M = 0;             // transforms per execute
     int chunk = 1;         // series per pass

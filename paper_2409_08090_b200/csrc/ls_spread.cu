@@ -163,6 +163,32 @@ struct PolyDeg<double> { static constexpr int value = 12; };
 template <>
 struct PolyDeg<float> { static constexpr int value = 8; };
 
+// Cells [lbase, lbase + CPT) of one thread += the staged candidates [pb, pe) (cell order); NR <= NS
+// rows are live.
+template <typename T, int NR, int NS, int CPT>
+__device__ __forceinline__ void gather_cells(typename V2<T>::type (&acc)[NS][CPT], const typename V2<T>::type* sc,
+                                             const T* sval, const int* srel, int pb, int pe, int lbase, int w) {
+    using T2 = typename V2<T>::type;
+    for (int pt = pb; pt < pe; ++pt) {
+        const int i0 = lbase - srel[pt];
+        T2 cs[NR];
+#pragma unroll
+        for (int s = 0; s < NR; ++s) cs[s] = sc[s * kChunkPts + pt];
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) {
+            const int i = i0 + c;
+            if ((unsigned)i < (unsigned)w) {
+                const T k = sval[i * kValStride + pt];
+#pragma unroll
+                for (int s = 0; s < NR; ++s) {
+                    acc[s][c].x = fma(k, cs[s].x, acc[s][c].x);
+                    acc[s][c].y = fma(k, cs[s].y, acc[s][c].y);
+                }
+            }
+        }
+    }
+}
+
 template <typename T, int NS, int CPT>
 __global__ void __launch_bounds__(kSpreadThreads, (NS * CPT <= 8) ? 4 : 3)
 ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
@@ -197,7 +223,10 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     // above n are the periodic images (shift -n / +n applied to the point's cell).
     const int lo = tile_lo - a.H, hi = tile_lo + Lt + a.H;
     int pbeg0, pcnt0, pbeg1 = 0, pcnt1 = 0, pcnt2 = 0;
-    {
+    if (lo >= 0 && hi <= a.n) {                      // interior tile: two loads, no images
+        pbeg0 = __ldg(&sg.bin_start[(unsigned)lo / kBinCells]);
+        pcnt0 = __ldg(&sg.bin_start[(unsigned)(hi - 1) / kBinCells + 1]) - pbeg0;
+    } else {
         const int mlo = max(lo, 0), mhi = min(hi, a.n);
         pbeg0 = __ldg(&sg.bin_start[mlo / kBinCells]);
         pcnt0 = __ldg(&sg.bin_start[(mhi - 1) / kBinCells + 1]) - pbeg0;
@@ -236,13 +265,12 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
                 }
                 int l0;
                 load_rec(sg.rec + g, eta, l0, qx, qy);
+                // strengths are fetched with the record, not after it: one global round trip, not two
+#pragma unroll
+                for (int s = 0; s < NS; ++s)
+                    if (s < nr) r[s] = __ldg(&sg.rows[(long long)(row0 + s) * a.Nd + g]);
                 rel = l0 + shift - tile_lo;          // first touched cell, tile-relative
                 have = rel + w > 0 && rel < Lt;
-                if (have) {
-#pragma unroll
-                    for (int s = 0; s < NS; ++s)
-                        if (s < nr) r[s] = __ldg(&sg.rows[(long long)(row0 + s) * a.Nd + g]);
-                }
             }
         }
         if (base == 0) {                             // later chunks find cnt re-zeroed by the scan
@@ -288,25 +316,10 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
         __syncthreads();
         // ---- 4. gather: cell l receives every point with rel in [l - w + 1, l], i.e. key in [l, l + w)
         if (lbase < Lt) {
-            const int pe = start[lbase + CPT - 1 + w];
-            for (int pt = start[lbase]; pt < pe; ++pt) {
-                const int i0 = lbase - srel[pt];
-                T2 cs[NS];
-#pragma unroll
-                for (int s = 0; s < NS; ++s) cs[s] = sc[s * kChunkPts + pt];
-#pragma unroll
-                for (int c = 0; c < CPT; ++c) {
-                    const int i = i0 + c;
-                    if ((unsigned)i < (unsigned)w) {
-                        const T k = sval[i * kValStride + pt];
-#pragma unroll
-                        for (int s = 0; s < NS; ++s) {
-                            acc[s][c].x = fma(k, cs[s].x, acc[s][c].x);
-                            acc[s][c].y = fma(k, cs[s].y, acc[s][c].y);
-                        }
-                    }
-                }
-            }
+            const int pb = start[lbase], pe = start[lbase + CPT - 1 + w];
+            // the x2 group of a single series carries one live row: skip the dead half of the FMAs
+            if (NS > 1 && nr == 1) gather_cells<T, 1, NS, CPT>(acc, sc, sval, srel, pb, pe, lbase, w);
+            else gather_cells<T, NS, NS, CPT>(acc, sc, sval, srel, pb, pe, lbase, w);
         }
         if (base + kChunkPts < total) __syncthreads();   // staging area is reused by the next chunk
     }
