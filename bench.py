@@ -54,6 +54,7 @@ def parse_args():
     ap.add_argument("--tile-cells", type=int, default=0)
     ap.add_argument("--upsampfac", type=float, default=0.0)
     ap.add_argument("--kernel-width", type=int, default=0)
+    ap.add_argument("--batch-chunk", type=int, default=0)
     return ap.parse_args()
 
 
@@ -227,7 +228,7 @@ def run_ours(args):
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     plan = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F64 if w.dtype == "f64" else B.LS_F32, w.batch,
                   timing=1, device=local, tile_cells=args.tile_cells, upsampfac=args.upsampfac,
-                  kernel_width=args.kernel_width)
+                  kernel_width=args.kernel_width, batch_chunk=args.batch_chunk)
     info = plan.info
     stream = torch.cuda.current_stream().cuda_stream
 

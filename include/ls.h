@@ -78,7 +78,7 @@ typedef struct {
     int timing;             /* 1: record CUDA events around each stage of every execute           */
     int device;             /* CUDA device ordinal the plan lives on                              */
     int tile_cells;         /* spreading tile length L in cells; 0 = auto                         */
-    int batch_chunk;        /* transforms spread/FFT'd/assembled per pass; 0 = auto (L2-sized)    */
+    int batch_chunk;        /* series spread/FFT'd/assembled per pass; 0 = auto (<= 8 GB of grids)  */
     int reserved[8];        /* must be zero                                                       */
 } ls_opts;
 

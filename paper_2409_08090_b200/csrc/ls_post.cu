@@ -56,8 +56,12 @@ struct AssembleArgs {
 //   C2w = |den|/r, S2w = num sign(den)/r, r = hypot(num, den)   [= 1/sqrt(1+tan^2), tan C2w]
 //   Sw  = S2w / (2 Cw)                                           [= sign(S2w) sqrt((1-C2w)/2)]
 // and the conventions of reading A14 for 0/0 and non-positive CC, SS.
-__device__ __forceinline__ double assemble_power(double Sh, double Ch, double S, double C, double S2, double C2,
-                                                 double inv_YY) {
+// Per-frequency part (depends on the weights only: shared by every series of a batch with common dy):
+// the rotation (Cw, Sw) = (cos, sin)(omega tau) and the reciprocals of CC, SS (0 where the term is dropped).
+struct FreqTerms {
+    double Cw, Sw, iCC, iSS;
+};
+__device__ __forceinline__ FreqTerms freq_terms(double S, double C, double S2, double C2) {
     const double num = S2 - 2.0 * S * C;
     const double den = C2 - (C * C - S * S);
     const double r = sqrt(num * num + den * den);
@@ -67,17 +71,25 @@ __device__ __forceinline__ double assemble_power(double Sh, double Ch, double S,
         C2w = fabs(den) * ir;
         S2w = (den < 0.0 ? -num : num) * ir;
     }
-    const double Cw = sqrt(0.5 * (1.0 + C2w));
-    const double Sw = S2w / (2.0 * Cw);
-    const double YC = Ch * Cw + Sh * Sw;
-    const double YS = Sh * Cw - Ch * Sw;
-    const double a = C * Cw + S * Sw, b = S * Cw - C * Sw;
+    FreqTerms f;
+    f.Cw = sqrt(0.5 * (1.0 + C2w));
+    f.Sw = S2w / (2.0 * f.Cw);
+    const double a = C * f.Cw + S * f.Sw, b = S * f.Cw - C * f.Sw;
     const double CC = 0.5 * (1.0 + C2 * C2w + S2 * S2w) - a * a;
     const double SS = 0.5 * (1.0 - C2 * C2w - S2 * S2w) - b * b;
-    double P = 0.0;
-    if (CC > 0.0) P += YC * YC / CC;
-    if (SS > 0.0) P += YS * YS / SS;
-    return P * inv_YY;
+    f.iCC = CC > 0.0 ? 1.0 / CC : 0.0;
+    f.iSS = SS > 0.0 ? 1.0 / SS : 0.0;
+    return f;
+}
+// Per-series part: YC, YS in the rotated frame and the standard-normalised power.
+__device__ __forceinline__ double series_power(const FreqTerms& f, double Sh, double Ch, double inv_YY) {
+    const double YC = Ch * f.Cw + Sh * f.Sw;
+    const double YS = Sh * f.Cw - Ch * f.Sw;
+    return (YC * YC * f.iCC + YS * YS * f.iSS) * inv_YY;
+}
+__device__ __forceinline__ double assemble_power(double Sh, double Ch, double S, double C, double S2, double C2,
+                                                 double inv_YY) {
+    return series_power(freq_terms(S, C, S2, C2), Sh, Ch, inv_YY);
 }
 
 template <typename T>
@@ -99,6 +111,33 @@ ls_assemble_kernel(const AssembleArgs a) {
     const double P = assemble_power((double)gh.y * d, (double)gh.x * d, (double)gw.y * d, (double)gw.x * d,
                                     (double)g2.y * d, (double)g2.x * d, 1.0 / YY);
     reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k] = (T)P;
+}
+
+// Batch with shared dy: the (w, w2) transforms and hence FreqTerms are common to all series, so one
+// thread owns a frequency, computes them once and streams kSeriesPerThread series' h-modes through.
+constexpr int kSeriesPerThread = 16;
+template <typename T>
+__global__ void __launch_bounds__(kPostThreads)
+ls_assemble_shared_kernel(const AssembleArgs a, int nseries) {
+    using T2 = typename V2<T>::type;
+    const long long k = (long long)blockIdx.x * kPostThreads + threadIdx.x;
+    if (k >= a.Nf) return;
+    const long long kp = k - a.half;
+    const long long idx = kp < 0 ? kp + a.n : kp;
+    const double d = a.dinv[kp < 0 ? -kp : kp];
+    const T2* g = reinterpret_cast<const T2*>(a.grids);
+    const T2 gw = g[(long long)a.w_slot * a.n + idx];
+    const T2 g2 = g[(long long)a.w2_slot * a.n + idx];
+    const FreqTerms f = freq_terms((double)gw.y * d, (double)gw.x * d, (double)g2.y * d, (double)g2.x * d);
+    const int i0 = blockIdx.y * kSeriesPerThread;
+    const int i1 = min(i0 + kSeriesPerThread, nseries);
+#pragma unroll 4
+    for (int i = i0; i < i1; ++i) {
+        const int s = a.series0 + i;
+        const T2 gh = __ldcs(&g[(long long)(a.h_slot + i) * a.n + idx]);
+        const double P = series_power(f, (double)gh.y * d, (double)gh.x * d, 1.0 / a.sums[4 * s + 2]);
+        __stcs(&reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k], (T)P);
+    }
 }
 
 template <typename T>
@@ -144,9 +183,16 @@ cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, 
     a.w_slot = w_slot; a.w_stride = w_stride;
     a.w2_slot = w2_slot; a.w2_stride = w2_stride;
     a.power = power;
-    dim3 grid((unsigned)((p->Nf + kPostThreads - 1) / kPostThreads), nseries);
-    if (p->dtype == LS_F64) ls_assemble_kernel<double><<<grid, kPostThreads, 0, s>>>(a);
-    else ls_assemble_kernel<float><<<grid, kPostThreads, 0, s>>>(a);
+    const unsigned gx = (unsigned)((p->Nf + kPostThreads - 1) / kPostThreads);
+    if (nseries > 1 && h_stride == 1 && w_stride == 0 && w2_stride == 0) {       // shared dy
+        dim3 grid(gx, (nseries + kSeriesPerThread - 1) / kSeriesPerThread);
+        if (p->dtype == LS_F64) ls_assemble_shared_kernel<double><<<grid, kPostThreads, 0, s>>>(a, nseries);
+        else ls_assemble_shared_kernel<float><<<grid, kPostThreads, 0, s>>>(a, nseries);
+    } else {
+        dim3 grid(gx, nseries);
+        if (p->dtype == LS_F64) ls_assemble_kernel<double><<<grid, kPostThreads, 0, s>>>(a);
+        else ls_assemble_kernel<float><<<grid, kPostThreads, 0, s>>>(a);
+    }
     return cudaGetLastError();
 }
 
