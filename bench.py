@@ -150,7 +150,7 @@ def time_oracle(w, K):
 
 def config_dict(w, extra=None):
     d = {"workload": w.name, "Nd": w.Nd, "Nf": w.Nf, "batch": w.batch, "eps": w.eps,
-         "l2": "flushed between steps (write of a 512 MiB buffer); grids (>= 3 x 400 MB at config 3) exceed L2 anyway"}
+         "l2": "flushed between steps (write of a 512 MiB buffer, > the 126 MB L2)"}
     if extra:
         d.update(extra)
     return d
@@ -190,16 +190,38 @@ STAGE_BYTES_DOC = "DESIGN.md §6"
 
 
 def stage_model_bytes(w, info):
-    """Algorithmic HBM bytes per execute of each own stage."""
+    """Algorithmic HBM bytes per execute of each own stage: every
+    intermediate written once and read once, nothing counted for re-reads or halo candidates."""
     B = 8 if w.dtype == "f64" else 4
     Nd, Nf, n, M, batch = w.Nd, w.Nf, info["n"], info["M"], w.batch
+    nbins = n // 64
+    rec = 4 * B                                           # one bin-sorted point record (32 B fp64 / 16 B fp32)
+    rows = M * Nd * B                                     # real strengths, one row per transform
     return {
-        "stats": batch * Nd * B + Nd * B,
-        "sort": 8 * Nd + 2 * 4 * (n // 256),
-        "premul": 8 * Nd + batch * Nd * B + Nd * B + 2 * Nd * (4 + B + 2 * B) + (M) * Nd * B,
-        "spread": M * n * 2 * B + 2 * Nd * (4 + B + 2 * B) + M * Nd * B,
+        "stats": 8 * Nd + batch * Nd * B + Nd * B + 2 * 4 * nbins,
+        "sort": 3 * 2 * 4 * nbins,
+        "premul": 8 * Nd + batch * Nd * B + Nd * B + 2 * Nd * rec + rows + (0 if batch == 1 else 2 * 4 * Nd),
+        "spread": M * n * 2 * B + 2 * Nd * rec + rows,
         "assemble": M * Nf * 2 * B + batch * Nf * B + (Nf // 2 + 1) * 8,
     }
+
+
+def measured_traffic(kernel_stage, w, info):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
+    ncu --set full capture (profiles/r1c_traffic.csv; same command line, config 3 defaults).  None when
+    the capture does not cover this workload / plan."""
+    path = os.path.join(ROOT, "profiles", "r1c_traffic.csv")
+    try:
+        with open(path) as f:
+            rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
+        hdr, rows = rows[0], rows[1:]
+        for r in rows:
+            d = dict(zip(hdr, r))
+            if d["stage"] == kernel_stage and d["workload"] == w.name and int(d["n"]) == info["n"] and int(d["w"]) == info["w"]:
+                return float(d["dram_read_bytes"]) + float(d["dram_write_bytes"])
+    except Exception:
+        pass
+    return None
 
 
 def run_ours(args):
@@ -310,7 +332,7 @@ def run_ours(args):
         "stage_ms": stage, "wall_ms_per_step_incl_flush": wall / args.steps * 1e3,
         "step_ms_min": float(np.min(step_ms)), "step_ms_median": float(np.median(step_ms)),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                     "traffic": None, "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
+                     "traffic": measured_traffic(dom, w, info), "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
                      "kernel_ms": stage[dom]},
         "path_roofline": {"what": "all own kernels (total - cuFFT), model bytes of " + STAGE_BYTES_DOC,
                           "bytes": info["model_bytes"], "ms": path_ms, "achieved": path_ach, "unit": "GB/s",
