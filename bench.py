@@ -185,6 +185,25 @@ def run_reference(args):
     print(json.dumps(line), flush=True)
 
 
+# ----------------------------------------------------------------------------- multi-rank host logic
+def max_over_ranks(values, device, world):
+    """Element-wise MAX over all ranks of a list of per-rank timings (the contract's max-over-ranks);
+    identity at world size 1.  Works on any backend (NCCL on the GPU box, gloo in the CPU tests)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+def whole_job_value(total_ms, steps, batch, world):
+    """(ms per step, ms per periodogram) of the WHOLE job: every rank runs `batch` periodograms per step
+    (weak scaling: no exchange step), all ranks' periodograms divide the slowest rank's time."""
+    ms_per_step = total_ms / steps
+    return ms_per_step, ms_per_step / (batch * world)
+
+
 # ----------------------------------------------------------------------------- our arm
 STAGE_BYTES_DOC = "DESIGN.md §6"
 
@@ -299,18 +318,14 @@ def run_ours(args):
     barrier()
     clocks = sampler.stop() if rank == 0 else None      # sampled over both timed legs
 
-    tmax = torch.tensor([dev_ms, e2e_ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    dev_ms, e2e_ms = float(tmax[0]), float(tmax[1])
+    dev_ms, e2e_ms = max_over_ranks([dev_ms, e2e_ms], dev, world)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
 
     n_periodograms = w.batch * world                      # per step, all ranks
-    ms_per_step = dev_ms / args.steps
-    value = ms_per_step / n_periodograms
+    ms_per_step, value = whole_job_value(dev_ms, args.steps, w.batch, world)
     stage = {k: v / args.steps for k, v in stage_acc.items()}
     peak, peak_src = measured_peak()
     sbytes = stage_model_bytes(w, info)
