@@ -79,7 +79,10 @@ typedef struct {
     int device;             /* CUDA device ordinal the plan lives on                              */
     int tile_cells;         /* spreading tile length L in cells; 0 = auto                         */
     int batch_chunk;        /* series spread/FFT'd/assembled per pass; 0 = auto (<= 8 GB of grids)  */
-    int reserved[8];        /* must be zero                                                       */
+    int no_autotune;        /* 1: never time candidate grid sizes at plan time (auto n = power of two) */
+    int graph;              /* 0 = auto: small problems replay a captured CUDA graph when timing == 0;
+                               1 = never, 2 = always (when timing == 0)                            */
+    int reserved[6];        /* must be zero                                                       */
 } ls_opts;
 
 /* ls_plan — choose (sigma, w, beta, n) from eps ("width and fine grid size are

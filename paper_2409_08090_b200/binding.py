@@ -35,7 +35,9 @@ class ls_opts(C.Structure):
         ("device", C.c_int),
         ("tile_cells", C.c_int),
         ("batch_chunk", C.c_int),
-        ("reserved", C.c_int * 8),
+        ("no_autotune", C.c_int),
+        ("graph", C.c_int),
+        ("reserved", C.c_int * 6),
     ]
 
 

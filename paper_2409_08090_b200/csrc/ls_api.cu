@@ -140,6 +140,70 @@ void fit_kernel_poly(int w, double beta, double tol, int max_deg, lsb::KernelPol
     *kp = best;
 }
 
+// Autotuned grid size, used when the power-of-two grid would be much larger than needed (sigma > 1.6;
+// measured at config 5: 3 x 2^28 C2C 10.1 ms, 3 x 1.6e8 6.3 ms).  cuFFT's time follows its pass structure
+// rather than n, so the few smallest {2,3,5}-smooth sizes >= 1.25 Nf, 3*2^k and 5*2^k are TIMED (three
+// transforms, scratch data) and the cheapest by  t_fft + own-kernel grid traffic  is taken.
+int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2) {
+    const cufftType type = dtype == LS_F64 ? CUFFT_Z2Z : CUFFT_C2C;
+    const size_t cell = dtype == LS_F64 ? 16 : 8;
+    std::vector<int64_t> cand;
+    cand.push_back(n_pow2);
+    const int64_t lo = (int64_t)ceil(1.25 * (double)Nf);
+    int64_t m = lo;
+    for (int i = 0; i < 5; ++i) {                      // the five smallest smooth sizes
+        m = next_smooth_even(m);
+        if (m >= n_pow2) break;
+        cand.push_back(m);
+        m += 4;
+    }
+    for (int64_t f : {3, 5}) {                         // few-pass sizes: 3 * 2^k, 5 * 2^k
+        int64_t v = f * 4;
+        while (v < lo) v *= 2;
+        if (v < n_pow2 && std::find(cand.begin(), cand.end(), v) == cand.end()) cand.push_back(v);
+    }
+    if (cand.size() == 1) return n_pow2;
+    void* buf = nullptr;
+    if (cudaMalloc(&buf, (size_t)n_pow2 * cell * 3) != cudaSuccess) { cudaGetLastError(); return n_pow2; }
+    cudaMemset(buf, 0, (size_t)n_pow2 * cell * 3);
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0);
+    cudaEventCreate(&e1);
+    int64_t best = n_pow2;
+    double best_cost = 1e300;
+    for (int64_t n : cand) {
+        cufftHandle h;
+        if (cufftCreate(&h) != CUFFT_SUCCESS) continue;
+        long long nn[1] = {(long long)n};
+        size_t ws = 0;
+        void* work = nullptr;
+        bool ok = cufftSetAutoAllocation(h, 0) == CUFFT_SUCCESS &&
+                  cufftMakePlanMany64(h, 1, nn, nullptr, 1, n, nullptr, 1, n, type, 3, &ws) == CUFFT_SUCCESS &&
+                  cudaMalloc(&work, ws ? ws : 16) == cudaSuccess && cufftSetWorkArea(h, work) == CUFFT_SUCCESS;
+        float ms = 0;
+        if (ok) {
+            for (int it = 0; it < 3 && ok; ++it) {      // two warm-ups, the third is timed
+                if (it == 2) cudaEventRecord(e0, 0);
+                ok = (dtype == LS_F64 ? cufftExecZ2Z(h, (cufftDoubleComplex*)buf, (cufftDoubleComplex*)buf, CUFFT_INVERSE)
+                                      : cufftExecC2C(h, (cufftComplex*)buf, (cufftComplex*)buf, CUFFT_INVERSE)) == CUFFT_SUCCESS;
+            }
+            cudaEventRecord(e1, 0);
+            ok = ok && cudaEventSynchronize(e1) == cudaSuccess && cudaEventElapsedTime(&ms, e0, e1) == cudaSuccess;
+        }
+        cufftDestroy(h);
+        cudaFree(work);
+        cudaGetLastError();
+        if (!ok) continue;
+        // own kernels: the grids are written once (spread, ~3.5 TB/s effective); the modes read do not depend on n
+        const double cost = ms + 3.0 * (double)n * cell / 3.5e9;
+        if (cost < best_cost) { best_cost = cost; best = n; }
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(buf);
+    return best;
+}
+
 template <typename T>
 cudaError_t dmalloc(ls_plan_s* p, T** ptr, size_t bytes) {
     if (bytes == 0) bytes = 16;
@@ -223,6 +287,7 @@ const char* ls_strerror(int code) {
 
 int ls_destroy(ls_plan_t p) {
     if (!p) return LS_OK;
+    if (p->gexec) cudaGraphExecDestroy(p->gexec);
     if (p->has_first) cufftDestroy(p->fft_first);
     if (p->has_chunk) cufftDestroy(p->fft_chunk);
     if (p->has_rem) cufftDestroy(p->fft_rem);
@@ -267,7 +332,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
                               o.tile_cells > lsb::kSpreadThreads * 4))
         return LS_ERR_INVALID_VALUE;
-    if (o.batch_chunk < 0) return LS_ERR_INVALID_VALUE;
+    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2) return LS_ERR_INVALID_VALUE;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || o.device < 0 || o.device >= ndev) return LS_ERR_CUDA;
@@ -296,6 +361,8 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         int64_t m = 64;                                 // >= 2 kMaxWidth
         while ((double)m < want) m *= 2;
         p->n = m;
+        if ((double)m > 1.6 * (double)Nf && m >= ((int64_t)1 << 20) && !o.no_autotune)
+            p->n = autotune_grid_size(Nf, dtype, m);
     }
     if (p->n >= ((int64_t)1 << 31) - 4096) { delete p; return LS_ERR_UNSUPPORTED; }
     p->sigma = (double)p->n / (double)Nf;
@@ -338,6 +405,8 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
 
     p->model_bytes = 8.0 * Nd + (double)batch * Nd * B + (per ? (double)batch : 1.0) * Nd * B + 8.0 * Nd +
                      (double)p->M * p->n * 2 * B + (double)p->M * Nf * 2 * B + (double)batch * Nf * B;
+
+    p->use_graph = !o.timing && (o.graph == 2 || (o.graph == 0 && p->model_bytes < 256e6));
 
     int rc = LS_OK;
     cudaError_t ce = cudaSuccess;
@@ -411,9 +480,8 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     return LS_OK;
 }
 
-int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, void* cuda_stream) {
-    if (!p || !t || !y || !dy || !power) return LS_ERR_INVALID_VALUE;
-    cudaStream_t s = (cudaStream_t)cuda_stream;
+// Enqueue the whole stage sequence on stream s (directly, or into a stream capture).
+static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, cudaStream_t s) {
     const bool per = p->opts.dy_per_series != 0;
     int own = 0, ffts = 0;
     cudaError_t ce = cudaSuccess;
@@ -492,6 +560,34 @@ int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* 
     p->fft_execs = ffts;
     return LS_OK;
 #undef LS_TRY
+}
+
+int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, void* cuda_stream) {
+    if (!p || !t || !y || !dy || !power) return LS_ERR_INVALID_VALUE;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // Small problems are launch-latency-bound ("GPU overheads"): replay the sequence as one graph.
+    // A legacy default stream cannot be captured; any capture failure falls back to direct launches for good.
+    if (!p->use_graph || s == nullptr) return enqueue_execute(p, t, y, dy, power, s);
+    if (!p->gexec || p->g_t != t || p->g_y != y || p->g_dy != dy || p->g_power != power) {
+        if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }
+        cudaGraph_t graph = nullptr;
+        int rc = LS_ERR_CUDA;
+        if (cudaStreamBeginCapture(s, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+            rc = enqueue_execute(p, t, y, dy, power, s);
+            if (cudaStreamEndCapture(s, &graph) != cudaSuccess || !graph) rc = LS_ERR_CUDA;
+            if (rc == LS_OK && cudaGraphInstantiate(&p->gexec, graph, 0) != cudaSuccess) rc = LS_ERR_CUDA;
+            if (graph) cudaGraphDestroy(graph);
+        }
+        if (rc != LS_OK) {
+            cudaGetLastError();
+            p->gexec = nullptr;
+            p->use_graph = false;
+            return enqueue_execute(p, t, y, dy, power, s);
+        }
+        p->g_t = t; p->g_y = y; p->g_dy = dy; p->g_power = power;
+    }
+    if (cudaGraphLaunch(p->gexec, s) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    return LS_OK;
 }
 
 int ls_execute_host(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, void* cuda_stream) {

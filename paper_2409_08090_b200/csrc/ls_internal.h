@@ -105,6 +105,11 @@ struct ls_plan_s {
     void* fft_work = nullptr;
     size_t fft_work_bytes = 0;
     size_t total_bytes = 0;
+    // CUDA-graph replay of the execute sequence (launch-latency-bound small problems; opts.graph)
+    bool use_graph = false;
+    cudaGraphExec_t gexec = nullptr;
+    const void *g_t = nullptr, *g_y = nullptr, *g_dy = nullptr;
+    void* g_power = nullptr;
     // timing
     std::vector<lsb::StageEvent> events;
     size_t events_used = 0;

@@ -16,7 +16,7 @@ def require_cuda():
     return torch
 
 
-def gpu_power(w, host=False, return_plan_info=False, debug_modes=None, **opts):
+def gpu_power(w, host=False, return_plan_info=False, debug_modes=None, side_stream=False, repeat=1, **opts):
     """P[batch, Nf] (float64 numpy) of Workload `w` via ls_plan / ls_execute(/_host) / ls_destroy."""
     torch = require_cuda()
     from paper_2409_08090_b200 import binding as B
@@ -26,7 +26,8 @@ def gpu_power(w, host=False, return_plan_info=False, debug_modes=None, **opts):
     plan = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F64 if w.dtype == "f64" else B.LS_F32, w.batch,
                   dy_per_series=dy_per, **opts)
     try:
-        stream = torch.cuda.current_stream().cuda_stream
+        sobj = torch.cuda.Stream() if side_stream else torch.cuda.current_stream()
+        stream = sobj.cuda_stream
         if host:
             P = np.empty((w.batch, w.Nf), dtype=w.np_dtype)
             plan.execute_host(np.ascontiguousarray(w.t), np.ascontiguousarray(w.y), np.ascontiguousarray(w.dy), P, stream)
@@ -36,7 +37,13 @@ def gpu_power(w, host=False, return_plan_info=False, debug_modes=None, **opts):
             y = torch.from_numpy(np.ascontiguousarray(w.y)).to(dev)
             dy = torch.from_numpy(np.ascontiguousarray(w.dy)).to(dev)
             P = torch.full((w.batch, w.Nf), float("nan"), dtype=tdt, device=dev)
-            plan.execute(t, y, dy, P, stream)
+            torch.cuda.synchronize()
+            for _ in range(repeat):                      # same buffers: a graph plan replays its capture
+                plan.execute(t, y, dy, P, stream)
+            if repeat > 1:                               # new output buffer: the plan must notice and re-capture
+                P = torch.full((w.batch, w.Nf), float("nan"), dtype=tdt, device=dev)
+                torch.cuda.synchronize()
+                plan.execute(t, y, dy, P, stream)
             torch.cuda.synchronize()
             out = P.cpu().numpy().astype(np.float64)
         extra = {}

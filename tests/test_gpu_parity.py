@@ -176,6 +176,40 @@ def test_execute_host_matches_device():
     assert np.max(np.abs(gpu_power(w5) - gpu_power(w5, host=True))) <= 1e-5
 
 
+def test_graph_replay_matches_direct_launches():
+    """opts.graph = 2 on a side stream: capture once, replay, re-capture when a buffer changes; identical
+    to direct launches (graph = 1)."""
+    w = scaled_workload(2, 3000)
+    P_direct = gpu_power(w, graph=1, side_stream=True)
+    P_graph = gpu_power(w, graph=2, side_stream=True, repeat=3)
+    assert np.max(np.abs(P_graph - P_direct)) <= 1e-13
+    P_auto_legacy = gpu_power(w)                       # auto mode on the legacy default stream: direct launches
+    assert np.max(np.abs(P_auto_legacy - P_direct)) <= 1e-13
+    _check64(errors(P_graph[0], oracle_power(w, fast=True)), pointwise=False)
+    wb = scaled_workload(4, 1200, batch=5)              # batch path through a graph
+    assert np.max(np.abs(gpu_power(wb, graph=2, side_stream=True, repeat=2) - gpu_power(wb, graph=1))) <= 1e-13
+
+
+def test_autotuned_grid_size():
+    """N_f just above a power of two / 1.6: the plan times candidate grid sizes and may take a
+    non-power-of-two n; whatever it takes must meet the gate, and no_autotune must give the power of two."""
+    rng = np.random.default_rng(77)
+    Nd, Nf = 20_000, 650_000                            # 1.25 Nf = 812 500 -> 2^20 has sigma 1.61
+    t = rng.uniform(0, 500, Nd)
+    dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    y = np.sin(2 * np.pi * 40000.3 * df * t) + rng.normal(0, 0.5, Nd)
+    w = _custom(t, y, dy, df, df, Nf)
+    ks = np.unique(np.concatenate([compare_indices(w, 600), np.arange(39990, 40010)]))   # incl. the peak
+    Po = oracle_power(w, ks=ks)
+    Pa, exa = gpu_power(w, return_plan_info=True)
+    Pp, exp_ = gpu_power(w, return_plan_info=True, no_autotune=1)
+    assert exp_["info"]["n"] == 1 << 20
+    assert 1.25 * Nf <= exa["info"]["n"] <= 1 << 20 and exa["info"]["n"] % 4 == 0
+    _check64(errors(Pa[0][ks], Po))
+    _check64(errors(Pp[0][ks], Po))
+
+
 def test_repeat_execute_is_stable():
     """Tile-owner spreading uses no floating-point atomics on the grid: repeated executes of one plan
     agree to rounding of the (atomic) statistics sums."""
