@@ -55,6 +55,7 @@ def parse_args():
     ap.add_argument("--upsampfac", type=float, default=0.0)
     ap.add_argument("--kernel-width", type=int, default=0)
     ap.add_argument("--batch-chunk", type=int, default=0)
+    ap.add_argument("--fft-impl", type=int, default=0, help="0 auto, 1 cuFFT, 2 own three-pass FFT")
     return ap.parse_args()
 
 
@@ -268,7 +269,7 @@ def run_ours(args):
     hP = torch.empty((w.batch, w.Nf), dtype=tdt).pin_memory()
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     popts = dict(device=local, tile_cells=args.tile_cells, upsampfac=args.upsampfac,
-                 kernel_width=args.kernel_width, batch_chunk=args.batch_chunk)
+                 kernel_width=args.kernel_width, batch_chunk=args.batch_chunk, fft_impl=args.fft_impl)
     ldt = B.LS_F64 if w.dtype == "f64" else B.LS_F32
     # Two plans: `plan` is what a user runs (no stage events; small problems replay a CUDA graph) and gives
     # `value`; `plan_t` records CUDA events around every stage and gives stage_ms / the roofline legs.

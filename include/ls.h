@@ -82,7 +82,9 @@ typedef struct {
     int no_autotune;        /* 1: never time candidate grid sizes at plan time (auto n = power of two) */
     int graph;              /* 0 = auto: small problems replay a captured CUDA graph when timing == 0;
                                1 = never, 2 = always (when timing == 0)                            */
-    int reserved[6];        /* must be zero                                                       */
+    int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs a
+                               2^24-cell fp64 grid; LS_ERR_UNSUPPORTED otherwise)                   */
+    int reserved[5];        /* must be zero                                                       */
 } ls_opts;
 
 /* ls_plan — choose (sigma, w, beta, n) from eps ("width and fine grid size are

@@ -37,7 +37,8 @@ class ls_opts(C.Structure):
         ("batch_chunk", C.c_int),
         ("no_autotune", C.c_int),
         ("graph", C.c_int),
-        ("reserved", C.c_int * 6),
+        ("fft_impl", C.c_int),
+        ("reserved", C.c_int * 5),
     ]
 
 

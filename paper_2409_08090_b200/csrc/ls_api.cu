@@ -144,7 +144,7 @@ void fit_kernel_poly(int w, double beta, double tol, int max_deg, lsb::KernelPol
 // measured at config 5: 3 x 2^28 C2C 10.1 ms, 3 x 1.6e8 6.3 ms).  cuFFT's time follows its pass structure
 // rather than n, so the few smallest {2,3,5}-smooth sizes >= 1.25 Nf, 3*2^k and 5*2^k are TIMED (three
 // transforms, scratch data) and the cheapest by  t_fft + own-kernel grid traffic  is taken.
-int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2) {
+int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2, int ntrans) {
     const cufftType type = dtype == LS_F64 ? CUFFT_Z2Z : CUFFT_C2C;
     const size_t cell = dtype == LS_F64 ? 16 : 8;
     std::vector<int64_t> cand;
@@ -164,8 +164,10 @@ int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2) {
     }
     if (cand.size() == 1) return n_pow2;
     void* buf = nullptr;
-    if (cudaMalloc(&buf, (size_t)n_pow2 * cell * 3) != cudaSuccess) { cudaGetLastError(); return n_pow2; }
-    cudaMemset(buf, 0, (size_t)n_pow2 * cell * 3);
+    // time with as many transforms as one execute pass has, capped so that the scratch stays <= 1 GB
+    const int nb = (int)std::max<size_t>(3, std::min<size_t>((size_t)ntrans, ((size_t)1 << 30) / ((size_t)n_pow2 * cell)));
+    if (cudaMalloc(&buf, (size_t)n_pow2 * cell * nb) != cudaSuccess) { cudaGetLastError(); return n_pow2; }
+    cudaMemset(buf, 0, (size_t)n_pow2 * cell * nb);
     cudaEvent_t e0, e1;
     cudaEventCreate(&e0);
     cudaEventCreate(&e1);
@@ -178,7 +180,7 @@ int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2) {
         size_t ws = 0;
         void* work = nullptr;
         bool ok = cufftSetAutoAllocation(h, 0) == CUFFT_SUCCESS &&
-                  cufftMakePlanMany64(h, 1, nn, nullptr, 1, n, nullptr, 1, n, type, 3, &ws) == CUFFT_SUCCESS &&
+                  cufftMakePlanMany64(h, 1, nn, nullptr, 1, n, nullptr, 1, n, type, nb, &ws) == CUFFT_SUCCESS &&
                   cudaMalloc(&work, ws ? ws : 16) == cudaSuccess && cufftSetWorkArea(h, work) == CUFFT_SUCCESS;
         float ms = 0;
         if (ok) {
@@ -195,7 +197,7 @@ int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2) {
         cudaGetLastError();
         if (!ok) continue;
         // own kernels: the grids are written once (spread, ~3.5 TB/s effective); the modes read do not depend on n
-        const double cost = ms + 3.0 * (double)n * cell / 3.5e9;
+        const double cost = ms + (double)nb * (double)n * cell / 3.5e9;
         if (cost < best_cost) { best_cost = cost; best = n; }
     }
     cudaEventDestroy(e0);
@@ -294,6 +296,9 @@ int ls_destroy(ls_plan_t p) {
     cudaFree(p->fft_work);
     cudaFree(p->grids);
     cudaFree(p->dinv);
+    cudaFree(p->fft_wlo);
+    cudaFree(p->fft_whi);
+    cudaFree(p->modes);
     cudaFree(p->zeroed);                     // sums and both histograms live in this allocation
     cudaFree(p->scan_tmp);
     for (int i = 0; i < 2; ++i) {
@@ -332,7 +337,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
                               o.tile_cells > lsb::kSpreadThreads * 4))
         return LS_ERR_INVALID_VALUE;
-    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2) return LS_ERR_INVALID_VALUE;
+    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 2) return LS_ERR_INVALID_VALUE;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || o.device < 0 || o.device >= ndev) return LS_ERR_CUDA;
@@ -361,16 +366,22 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         int64_t m = 64;                                 // >= 2 kMaxWidth
         while ((double)m < want) m *= 2;
         p->n = m;
-        if ((double)m > 1.6 * (double)Nf && m >= ((int64_t)1 << 20) && !o.no_autotune)
-            p->n = autotune_grid_size(Nf, dtype, m);
+        const int ntrans = o.dy_per_series ? 3 * batch : batch + 2;
+        if ((double)m > 1.6 * (double)Nf && (double)m * ntrans >= (double)((int64_t)1 << 20) && !o.no_autotune)
+            p->n = autotune_grid_size(Nf, dtype, m, ntrans);
     }
     if (p->n >= ((int64_t)1 << 31) - 4096) { delete p; return LS_ERR_UNSUPPORTED; }
     p->sigma = (double)p->n / (double)Nf;
     int w = o.kernel_width;
     if (w == 0) {
-        const double s = std::min(p->sigma, 2.0);      // tiny Nf: n is floored at 2 kMaxWidth cells
-        w = (int)ceil(-log(eps) / (M_PI * sqrt(1.0 - 1.0 / s)) - 1e-9);
-        w += dtype == LS_F64 ? 2 : 1;
+        const double s = std::min(p->sigma, 2.0);      // tiny Nf: n is floored at 64 cells
+        const double rate = M_PI * sqrt(1.0 - 1.0 / s);
+        // Measured (single point, sup norm over its position): the ES kernel's error is
+        // ~ 30 exp(-w rate) for sigma in [1.25, 2].  fp64: aim a decade below eps so that a pointwise
+        // reading of the tolerance holds too (A8) — 12 cells at sigma = 2, 17 at 1.34, 19 at 1.25, for
+        // eps = 1e-9.  fp32: the grid's own rounding (6e-8) dominates early; the plain rule plus one cell.
+        if (dtype == LS_F64) w = (int)ceil((-log(eps) + log(300.0)) / rate - 1e-9);
+        else w = (int)ceil(-log(eps) / rate - 1e-9) + 1;
         w = std::max(2, std::min(lsb::kMaxWidth, w));
     }
     p->w = w;
@@ -399,6 +410,9 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     }
     p->slots = per ? 3 * p->chunk : 2 + p->chunk;
 
+    p->own_fft = o.fft_impl != 1 && lsb::own_fft_supported(p);
+    if (o.fft_impl == 2 && !p->own_fft) { delete p; return LS_ERR_UNSUPPORTED; }
+
     // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
     p->ndf = two_prod((double)p->n, df);
     p->fc = dd_add_d(two_prod((double)(Nf / 2), df), f0);
@@ -413,10 +427,19 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     do {
         if ((ce = dmalloc(p, &p->grids, (size_t)p->slots * grid_bytes)) != cudaSuccess) break;
         if ((ce = dmalloc(p, &p->dinv, (size_t)(Nf / 2 + 1) * 8)) != cudaSuccess) break;
+        if (p->own_fft) {
+            if ((ce = dmalloc(p, (char**)&p->fft_wlo, (size_t)4096 * 16)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, (char**)&p->fft_whi, (size_t)std::max<int64_t>(4096, p->n / 4096) * 16)) != cudaSuccess) break;
+            if ((ce = dmalloc(p, (char**)&p->modes, (size_t)p->slots * Nf * 16)) != cudaSuccess) break;
+            if ((ce = lsb::own_fft_init(p, 0)) != cudaSuccess) break;
+        }
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
-        p->zeroed_bytes = sums_bytes + (size_t)2 * p->nbins * 4;
+        const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
+        const size_t mask_bytes = p->own_fft ? (size_t)2 * (p->n / 256 / p->L) * 16 * 4 : 0;
+        p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
+        if (p->own_fft) p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes);
         p->sums = (double*)p->zeroed;
         p->ps[0].hist = (int*)((char*)p->zeroed + sums_bytes);
         p->ps[1].hist = p->ps[0].hist + p->nbins;
@@ -437,6 +460,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         std::vector<Pass> passes;
         build_passes(p, passes);
         size_t work = 0;
+        if (!p->own_fft) {
         p->first_batch = passes.front().fft_batch;
         if ((rc = make_fft(p, &p->fft_first, p->first_batch, &work)) != LS_OK) break;
         p->has_first = true;
@@ -458,6 +482,8 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         if (cufftSetWorkArea(p->fft_first, p->fft_work) != CUFFT_SUCCESS) { rc = LS_ERR_CUFFT; break; }
         if (p->has_chunk && cufftSetWorkArea(p->fft_chunk, p->fft_work) != CUFFT_SUCCESS) { rc = LS_ERR_CUFFT; break; }
         if (p->has_rem && cufftSetWorkArea(p->fft_rem, p->fft_work) != CUFFT_SUCCESS) { rc = LS_ERR_CUFFT; break; }
+        }
+        if (rc != LS_OK) break;
 
         // P0: deconvolution table on the device
         double hz[lsb::kQuadNodes], hw[lsb::kQuadNodes];
@@ -533,7 +559,12 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
             stage_end(p, s);
 
             stage_begin(p, LS_STAGE_FFT, s);
-            {
+            if (p->own_fft) {
+                // own three-pass FFT: pass 1 skips the tiles spreading flagged empty, pass 3 emits the kept modes
+                const int n_x2 = per ? ps.C : (ps.s0 == 0 ? 1 : 0);
+                LS_TRY(lsb::launch_own_fft(p, ps.fft_slot0, ps.fft_batch, n_x2, true, s));
+                own += 3;
+            } else {
                 cufftHandle h = find_fft(p, ps.fft_batch);
                 if (cufftSetStream(h, s) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
                 char* base = (char*)p->grids + (size_t)ps.fft_slot0 * p->n * 2 * real_bytes(p->dtype);

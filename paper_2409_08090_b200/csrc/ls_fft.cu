@@ -1,0 +1,297 @@
+// ls_fft.cu — the library's own fine-grid FFT for n = 2^24 complex128 grids (
+// PAPER.md:47 "use an equispaced FFT", :73 "the FFT time dominates").
+//
+//   B_k = sum_l b_l e^{+2 pi i k l / n}     (reading A7: the unnormalised inverse transform)
+//
+// Three radix-256 passes over n = R1 R2 R3 = 256^3, decimation in frequency:
+//   l = l1 R2 R3 + l2 R3 + l3,   k = k1 + R1 k2 + R1 R2 k3
+//   pass 1: FFT over l1 -> k1, times w_n^{k1 (l2 R3 + l3)};   in place, layout [k1][l2][l3]
+//   pass 2: FFT over l2 -> k2, times w_n^{R1 k2 l3};          in place, layout [k1][k2][l3]
+//   pass 3: FFT over l3 -> k3; the kept modes k' = k - floor(Nf/2) in [-floor(Nf/2), ceil(Nf/2)) go to a
+//           compact [M][Nf] array in frequency order (coalesced: 16 consecutive k1 per store)
+// This is the pass structure cuFFT itself uses at this size (three regular_fft_factor<256> launches,
+// profiles/r1c_cfg3.md); what the own version adds is what a library cannot know:
+//   * pass 1 skips the loads of tiles the spreading kernel flagged empty (60-80 % of every grid at
+//     df = 1/(5T)), and the spreading kernel no longer has to write those zeros;
+//   * pass 3 writes only the N_f kept modes, already centred, so the assembly reads a dense array.
+//
+// One CTA = 256 threads = one tile of 256 (transform dimension) x 16 (other dimension) points:
+// 16-point FFTs in registers (radix 4 x 4), one shared-memory exchange (conflict-free layouts),
+// 256-byte global segments on both sides.  Twiddles: w_256 from a shared table, w_n^e from two
+// 4096-entry tables (e = 4096 e_hi + e_lo) and a base/step recurrence along the thread's 16 outputs.
+#include "ls_internal.h"
+
+namespace lsb {
+namespace {
+
+constexpr int kFftThreads = 256;
+constexpr double kC1 = 0.92387953251128675613;   // cos(pi/8)
+constexpr double kS1 = 0.38268343236508977173;   // sin(pi/8)
+constexpr double kR2 = 0.70710678118654752440;   // sqrt(1/2)
+
+__device__ __forceinline__ double2 cadd(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 csub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 cmul(double2 a, double2 w) {
+    return make_double2(fma(a.x, w.x, -a.y * w.y), fma(a.x, w.y, a.y * w.x));
+}
+__device__ __forceinline__ double2 cmuli(double2 a) { return make_double2(-a.y, a.x); }   // a * i
+
+// X_k = sum_l x_l e^{+2 pi i k l / 4}, in place (a,b,c,d) -> (X0,X1,X2,X3)
+__device__ __forceinline__ void fft4(double2& a, double2& b, double2& c, double2& d) {
+    const double2 t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = cmuli(csub(b, d));
+    a = cadd(t0, t2);
+    b = cadd(t1, t3);
+    c = csub(t0, t2);
+    d = csub(t1, t3);
+}
+
+// 16-point transform X_k = sum_l x_l e^{+2 pi i k l / 16}, in place; X_k ends at position
+// pos16(k) = 4 (k & 3) + (k >> 2).
+__device__ __forceinline__ constexpr int pos16(int k) { return 4 * (k & 3) + (k >> 2); }
+__device__ __forceinline__ void fft16(double2 (&x)[16]) {
+#pragma unroll
+    for (int b = 0; b < 4; ++b) fft4(x[b], x[4 + b], x[8 + b], x[12 + b]);     // over a: x[4 ka + b] = z[b][ka]
+    // twiddle w_16^{b ka}
+    x[5] = cmul(x[5], make_double2(kC1, kS1));       // b=1, ka=1: m=1
+    x[6] = cmul(x[6], make_double2(kR2, kR2));       // b=2, ka=1: m=2
+    x[7] = cmul(x[7], make_double2(kS1, kC1));       // b=3, ka=1: m=3
+    x[9] = cmul(x[9], make_double2(kR2, kR2));       // b=1, ka=2: m=2
+    x[10] = cmuli(x[10]);                            // b=2, ka=2: m=4
+    x[11] = cmul(x[11], make_double2(-kR2, kR2));    // b=3, ka=2: m=6
+    x[13] = cmul(x[13], make_double2(kS1, kC1));     // b=1, ka=3: m=3
+    x[14] = cmul(x[14], make_double2(-kR2, kR2));    // b=2, ka=3: m=6
+    x[15] = cmul(x[15], make_double2(-kC1, -kS1));   // b=3, ka=3: m=9
+#pragma unroll
+    for (int ka = 0; ka < 4; ++ka) fft4(x[4 * ka], x[4 * ka + 1], x[4 * ka + 2], x[4 * ka + 3]);
+}
+
+struct FftArgs {
+    double2* grids;            // [ntrans][n] in place
+    long long n;
+    int R1, R2, R3;            // 256 each
+    const double2* wlo;        // w_n^x, x < 4096
+    const double2* whi;        // w_n^{4096 y}, y < n / 4096
+    // pass 1 pruning (see PointSet-independent `row_masks` in ls_internal.h): for point set s, spreading-tile
+    // column ct = (m >> tile_shift) and j = row & 15, bit i of row_masks[(s * ncoltiles + ct) * 16 + j] says
+    // that row 16 i + j of that column holds data; unset = never written by the spreading kernel = zeros.
+    const unsigned* row_masks;
+    int ncoltiles;
+    int set_of_trans_first;    // transforms [0, set_of_trans_first) belong to set 0 (x2), the rest to set 1 (x1)
+    int tile_shift;            // log2(spreading tile length)
+    // pass 3 output
+    double2* modes;            // [ntrans][Nf]
+    long long Nf, half;
+};
+
+__device__ __forceinline__ double2 twiddle_n(const FftArgs& a, unsigned e) {
+    const double2 lo = __ldg(&a.wlo[e & 4095u]);
+    const double2 hi = __ldg(&a.whi[(e & (unsigned)(a.n - 1)) >> 12]);
+    return cmul(lo, hi);
+}
+
+// w_256^m table in shared memory, one entry per thread
+__device__ __forceinline__ void fill_w256(double2* w256) {
+    double s, c;
+    sincospi((double)threadIdx.x / 128.0, &s, &c);
+    w256[threadIdx.x] = make_double2(c, s);
+}
+
+// Passes 1 and 2: the transform dimension is strided (stride = inner), 16 consecutive columns per CTA.
+// Data viewed as [outer][256][inner]; in place.  Inter-pass twiddle w_n^{k_r * m * outer}.
+__global__ void __launch_bounds__(kFftThreads, 2)
+ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
+    extern __shared__ __align__(16) unsigned char fsm[];
+    double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
+    double2* w256 = Y + 256 * 16;
+    fill_w256(w256);
+    const int c = threadIdx.x & 15, hi4 = threadIdx.x >> 4;
+    const long long m = (long long)blockIdx.x * 16 + c;      // column
+    const int o = blockIdx.y, tr = blockIdx.z;
+    double2* base = a.grids + (long long)tr * a.n + (long long)o * 256 * inner + m;
+
+    double2 x[16];
+    {
+        const int j = hi4;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = base[(long long)(16 * i + j) * inner];
+        fft16(x);
+        __syncthreads();                                     // w256 ready
+#pragma unroll
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * 16 + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+    }
+    __syncthreads();
+    {
+        const int ka = hi4;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * 16 + c];
+        fft16(x);
+        // k_r = ka + 16 kb;  twiddle exponent e = k_r * m * outer (mod n) = e0 + kb * de
+        const unsigned mm = (unsigned)m * (unsigned)outer;
+        double2 tw = twiddle_n(a, (unsigned)ka * mm);
+        const double2 st = twiddle_n(a, 16u * mm);
+#pragma unroll
+        for (int kb = 0; kb < 16; ++kb) {
+            base[(long long)(ka + 16 * kb) * inner] = cmul(x[pos16(kb)], tw);
+            tw = cmul(tw, st);
+        }
+    }
+}
+
+// Pass 1, pruned and persistent: outer = 1, inner = n / 256.  Each CTA walks column tiles (16 columns x 256
+// rows of one transform); the 16-bit liveness mask of the NEXT tile is fetched while the current one is in
+// flight, so the mask never sits on the critical path.  Dead rows are not loaded (they were never written).
+__global__ void __launch_bounds__(kFftThreads, 2)
+ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int ntiles_total) {
+    extern __shared__ __align__(16) unsigned char fsm[];
+    double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
+    double2* w256 = Y + 256 * 16;
+    fill_w256(w256);
+    const int c = threadIdx.x & 15, hi4 = threadIdx.x >> 4;
+    auto mask_of = [&](int tile) -> unsigned {
+        if (tile >= ntiles_total) return 0u;
+        const int tr = tile / tiles_per_trans;
+        const long long m0 = (long long)(tile - tr * tiles_per_trans) * 16;
+        const int set = tr < a.set_of_trans_first ? 0 : 1;
+        return __ldg(&a.row_masks[((long long)set * a.ncoltiles + (m0 >> a.tile_shift)) * 16 + hi4]);
+    };
+    int tile = blockIdx.x;
+    unsigned live = mask_of(tile);
+    __syncthreads();                                         // w256 ready
+    for (; tile < ntiles_total; tile += gridDim.x) {
+        const int tr = tile / tiles_per_trans;
+        const long long m = (long long)(tile - tr * tiles_per_trans) * 16 + c;
+        double2* base = a.grids + (long long)tr * a.n + m;
+        double2 x[16];
+        {
+            const int j = hi4;
+#pragma unroll
+            for (int i = 0; i < 16; ++i) {
+                x[i] = make_double2(0.0, 0.0);
+                if (live >> i & 1u) x[i] = base[(long long)(16 * i + j) * inner];
+            }
+            live = mask_of(tile + gridDim.x);                // prefetch: lands during this tile's work
+            fft16(x);
+#pragma unroll
+            for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * 16 + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+        }
+        __syncthreads();
+        {
+            const int ka = hi4;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * 16 + c];
+            fft16(x);
+            const unsigned mm = (unsigned)m;
+            double2 tw = twiddle_n(a, (unsigned)ka * mm);
+            const double2 st = twiddle_n(a, 16u * mm);
+#pragma unroll
+            for (int kb = 0; kb < 16; ++kb) {
+                base[(long long)(ka + 16 * kb) * inner] = cmul(x[pos16(kb)], tw);
+                tw = cmul(tw, st);
+            }
+        }
+        __syncthreads();                                     // Y is reused by the next tile
+    }
+}
+
+// Pass 3: the transform dimension (l3) is contiguous; the CTA takes 16 consecutive k1 at one k2, so that the
+// kept modes leave in runs of 16 consecutive frequencies.  Output: modes[tr][k], k = (kk + half) mod n < Nf,
+// kk = k1 + R1 k2 + R1 R2 k3 the stored mode index (= k' mod n).
+__global__ void __launch_bounds__(kFftThreads, 2)
+ls_fft_rows_kernel(const FftArgs a) {
+    extern __shared__ __align__(16) unsigned char fsm[];
+    double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][17] (padded: conflict-free both ways)
+    double2* w256 = Y + 256 * 17;
+    fill_w256(w256);
+    const int k1b = blockIdx.x * 16, k2 = blockIdx.y, tr = blockIdx.z;
+    const double2* src = a.grids + (long long)tr * a.n;
+    double2 x[16];
+    {
+        const int j = threadIdx.x & 15, c = threadIdx.x >> 4;
+        const double2* row = src + ((long long)(k1b + c) * a.R2 + k2) * a.R3;
+#pragma unroll
+        for (int i = 0; i < 16; ++i) x[i] = row[16 * i + j];
+        fft16(x);
+        __syncthreads();
+#pragma unroll
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * 17 + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+    }
+    __syncthreads();
+    {
+        const int c = threadIdx.x & 15, ka = threadIdx.x >> 4;
+#pragma unroll
+        for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * 17 + c];
+        fft16(x);
+        double2* out = a.modes + (long long)tr * a.Nf;
+        const long long kk0 = (long long)(k1b + c) + (long long)a.R1 * k2;
+        const long long r12 = (long long)a.R1 * a.R2;
+#pragma unroll
+        for (int kb = 0; kb < 16; ++kb) {
+            long long k = kk0 + r12 * (ka + 16 * kb) + a.half;
+            if (k >= a.n) k -= a.n;
+            if (k < a.Nf) out[k] = x[pos16(kb)];
+        }
+    }
+}
+
+__global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < 4096) {
+        double s, c;
+        sincospi(2.0 * (double)i / (double)n, &s, &c);
+        wlo[i] = make_double2(c, s);
+    }
+    if ((long long)i < n / 4096) {
+        double s, c;
+        sincospi(2.0 * (double)i * 4096.0 / (double)n, &s, &c);
+        whi[i] = make_double2(c, s);
+    }
+}
+
+constexpr size_t kColsSmem = sizeof(double2) * (256 * 16 + 256);
+constexpr size_t kRowsSmem = sizeof(double2) * (256 * 17 + 256);
+
+}  // namespace
+
+bool own_fft_supported(const ls_plan_s* p) { return p->dtype == LS_F64 && p->n == ((int64_t)1 << 24); }
+
+cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
+    const int cnt = (int)std::max<long long>(4096, p->n / 4096);
+    ls_fft_tables_kernel<<<(cnt + 255) / 256, 256, 0, s>>>((double2*)p->fft_wlo, (double2*)p->fft_whi, p->n);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(ls_fft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem);
+}
+
+// FFT of transforms [slot0, slot0 + ntrans) of the plan's grids; the first n_x2 of them belong to the x2
+// point set (pruning flags).  Kept modes land in p->modes[slot0 + i][0..Nf).
+cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, bool prune, cudaStream_t s) {
+    FftArgs a;
+    a.grids = (double2*)p->grids + (long long)slot0 * p->n;
+    a.n = p->n;
+    a.R1 = a.R2 = a.R3 = 256;
+    a.wlo = (const double2*)p->fft_wlo;
+    a.whi = (const double2*)p->fft_whi;
+    a.row_masks = p->row_masks;
+    a.ncoltiles = (int)(p->n / 256 / p->L);
+    a.set_of_trans_first = n_x2;
+    a.tile_shift = 0;
+    while ((1 << a.tile_shift) < p->L) ++a.tile_shift;
+    a.modes = (double2*)p->modes + (long long)slot0 * p->Nf;
+    a.Nf = p->Nf;
+    a.half = p->Nf / 2;
+    const long long inner1 = p->n / 256, inner2 = p->n / 65536;
+    dim3 g1((unsigned)(inner1 / 16), 1, ntrans), g2((unsigned)(inner2 / 16), 256, ntrans), g3(256 / 16, 256, ntrans);
+    if (prune) {
+        const int tiles_per_trans = (int)(inner1 / 16), total = tiles_per_trans * ntrans;
+        ls_fft_pass1_kernel<<<std::min(total, 2 * p->num_sms), kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total);
+    } else {
+        ls_fft_cols_kernel<<<g1, kFftThreads, kColsSmem, s>>>(a, 1, inner1);
+    }
+    ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, 256, inner2);
+    ls_fft_rows_kernel<<<g3, kFftThreads, kRowsSmem, s>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace lsb

@@ -7,13 +7,14 @@
 #include <cufft.h>
 #include <stdint.h>
 
+#include <algorithm>
 #include <vector>
 
 #include "../../include/ls.h"
 
 namespace lsb {
 
-constexpr int kMaxWidth = 18;        // widest spreading kernel supported (cells)
+constexpr int kMaxWidth = 20;        // widest spreading kernel supported (cells)
 constexpr int kBinCells = 64;        // sort-bin length in fine-grid cells (>= kMaxWidth/2 + 1)
 constexpr int kSpreadThreads = 256;  // threads per spreading CTA
 constexpr int kChunkPts = 256;       // candidates a spreading CTA stages per pass (one per thread)
@@ -105,6 +106,11 @@ struct ls_plan_s {
     void* fft_work = nullptr;
     size_t fft_work_bytes = 0;
     size_t total_bytes = 0;
+    // own FFT (ls_fft.cu): n = 2^24 fp64; opts.fft_impl
+    bool own_fft = false;
+    void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
+    void* modes = nullptr;                          // [slots][Nf] complex: kept modes in frequency order
+    unsigned* row_masks = nullptr;                  // [2][n/256/L][16] liveness bits for FFT pass 1 (in `zeroed`)
     // CUDA-graph replay of the execute sequence (launch-latency-bound small problems; opts.graph)
     bool use_graph = false;
     cudaGraphExec_t gexec = nullptr;
@@ -131,6 +137,10 @@ cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_
 cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int row0_x1, int nrows_x1,
                           int slot0_x1, cudaStream_t s);
 int spread_rows_per_group(const ls_plan_s* p);
+// ---- ls_fft.cu: own three-pass FFT (n = 2^24, fp64) ------------------------------------------
+bool own_fft_supported(const ls_plan_s* p);
+cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
+cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, bool prune, cudaStream_t s);
 // ---- ls_post.cu: P0 table, K5+K6 -----------------------------------------------------------
 cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double* weights, cudaStream_t s);
 cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,

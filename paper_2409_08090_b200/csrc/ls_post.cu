@@ -42,8 +42,10 @@ template <>
 struct V2<float> { using type = float2; };
 
 struct AssembleArgs {
-    const void* grids;
+    const void* grids;              // fine grids after the FFT, or (compact) the own FFT's [slots][Nf] mode array
     long long n, Nf;
+    long long stride;               // elements between transforms: n, or Nf when compact
+    int compact;                    // 1: mode k of a transform sits at index k
     long long half;                 // floor(Nf/2)
     const double* dinv;
     const double* sums;
@@ -101,12 +103,12 @@ ls_assemble_kernel(const AssembleArgs a) {
     const int i = blockIdx.y;                      // series within this pass
     const int s = a.series0 + i;
     const long long kp = k - a.half;               // centred mode k'
-    const long long idx = kp < 0 ? kp + a.n : kp;
+    const long long idx = a.compact ? k : (kp < 0 ? kp + a.n : kp);
     const double d = a.dinv[kp < 0 ? -kp : kp];
     const T2* g = reinterpret_cast<const T2*>(a.grids);
-    const T2 gh = __ldcs(&g[(long long)(a.h_slot + i * a.h_stride) * a.n + idx]);
-    const T2 gw = g[(long long)(a.w_slot + i * a.w_stride) * a.n + idx];
-    const T2 g2 = g[(long long)(a.w2_slot + i * a.w2_stride) * a.n + idx];
+    const T2 gh = __ldcs(&g[(long long)(a.h_slot + i * a.h_stride) * a.stride + idx]);
+    const T2 gw = g[(long long)(a.w_slot + i * a.w_stride) * a.stride + idx];
+    const T2 g2 = g[(long long)(a.w2_slot + i * a.w2_stride) * a.stride + idx];
     const double YY = a.sums[4 * s + 2];
     const double P = assemble_power((double)gh.y * d, (double)gh.x * d, (double)gw.y * d, (double)gw.x * d,
                                     (double)g2.y * d, (double)g2.x * d, 1.0 / YY);
@@ -123,35 +125,35 @@ ls_assemble_shared_kernel(const AssembleArgs a, int nseries) {
     const long long k = (long long)blockIdx.x * kPostThreads + threadIdx.x;
     if (k >= a.Nf) return;
     const long long kp = k - a.half;
-    const long long idx = kp < 0 ? kp + a.n : kp;
+    const long long idx = a.compact ? k : (kp < 0 ? kp + a.n : kp);
     const double d = a.dinv[kp < 0 ? -kp : kp];
     const T2* g = reinterpret_cast<const T2*>(a.grids);
-    const T2 gw = g[(long long)a.w_slot * a.n + idx];
-    const T2 g2 = g[(long long)a.w2_slot * a.n + idx];
+    const T2 gw = g[(long long)a.w_slot * a.stride + idx];
+    const T2 g2 = g[(long long)a.w2_slot * a.stride + idx];
     const FreqTerms f = freq_terms((double)gw.y * d, (double)gw.x * d, (double)g2.y * d, (double)g2.x * d);
     const int i0 = blockIdx.y * kSeriesPerThread;
     const int i1 = min(i0 + kSeriesPerThread, nseries);
 #pragma unroll 4
     for (int i = i0; i < i1; ++i) {
         const int s = a.series0 + i;
-        const T2 gh = __ldcs(&g[(long long)(a.h_slot + i) * a.n + idx]);
+        const T2 gh = __ldcs(&g[(long long)(a.h_slot + i) * a.stride + idx]);
         const double P = series_power(f, (double)gh.y * d, (double)gh.x * d, 1.0 / a.sums[4 * s + 2]);
         __stcs(&reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k], (T)P);
     }
 }
 
 template <typename T>
-__global__ void ls_debug_modes_kernel(const void* grids, long long n, long long half, const double* dinv,
+__global__ void ls_debug_modes_kernel(const void* grids, long long n, long long stride, int compact, long long half, const double* dinv,
                                       int h_slot, int w_slot, int w2_slot, long long K,
                                       const long long* kidx, double* out) {
     using T2 = typename V2<T>::type;
     const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= K) return;
     const long long kp = kidx[q] - half;
-    const long long idx = kp < 0 ? kp + n : kp;
+    const long long idx = compact ? kidx[q] : (kp < 0 ? kp + n : kp);
     const double d = dinv[kp < 0 ? -kp : kp];
     const T2* g = reinterpret_cast<const T2*>(grids);
-    const T2 gh = g[(long long)h_slot * n + idx], gw = g[(long long)w_slot * n + idx], g2 = g[(long long)w2_slot * n + idx];
+    const T2 gh = g[(long long)h_slot * stride + idx], gw = g[(long long)w_slot * stride + idx], g2 = g[(long long)w2_slot * stride + idx];
     double* o = out + 6 * q;
     o[0] = (double)gh.y * d; o[1] = (double)gh.x * d;
     o[2] = (double)gw.y * d; o[3] = (double)gw.x * d;
@@ -171,9 +173,11 @@ cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double*
 cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,
                             int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s) {
     AssembleArgs a;
-    a.grids = p->grids;
+    a.grids = p->own_fft ? p->modes : p->grids;
     a.n = p->n;
     a.Nf = p->Nf;
+    a.stride = p->own_fft ? p->Nf : p->n;
+    a.compact = p->own_fft ? 1 : 0;
     a.half = p->Nf / 2;
     a.dinv = p->dinv;
     a.sums = p->sums;
@@ -200,10 +204,10 @@ cudaError_t launch_debug_modes(ls_plan_s* p, int h_slot, int w_slot, int w2_slot
                                const int64_t* d_kidx, double* d_out, cudaStream_t s) {
     const int nb = (int)((K + 127) / 128);
     if (p->dtype == LS_F64)
-        ls_debug_modes_kernel<double><<<nb, 128, 0, s>>>(p->grids, p->n, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
+        ls_debug_modes_kernel<double><<<nb, 128, 0, s>>>(p->own_fft ? p->modes : p->grids, p->n, p->own_fft ? p->Nf : p->n, p->own_fft ? 1 : 0, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
                                                          K, (const long long*)d_kidx, d_out);
     else
-        ls_debug_modes_kernel<float><<<nb, 128, 0, s>>>(p->grids, p->n, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
+        ls_debug_modes_kernel<float><<<nb, 128, 0, s>>>(p->grids, p->n, p->n, 0, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
                                                         K, (const long long*)d_kidx, d_out);
     return cudaGetLastError();
 }

@@ -57,6 +57,9 @@ struct SpreadArgs {
     int ntiles, tile_stride;         // CTA b owns tile (b * tile_stride) mod ntiles
     int tile_mask;                   // ntiles - 1 when ntiles is a power of two, else -1
     int half;                        // ceil(w/2) stored polynomial pieces
+    int skip_empty;                  // own FFT: tiles without points are flagged, not zero-filled
+    unsigned* row_masks;             // own FFT: liveness bits of the written tiles (layout: ls_fft.cu FftArgs)
+    int ncoltiles, coltile_shift;    // tiles per FFT pass-1 row (n / 256 / L, a power of two) and its log2
     long long Nd;
     SpreadSeg<T> seg[2];             // blockIdx.y < seg[0].ngroups: x2 rows, else x1 rows
     T c[kHalfMax][kMaxDeg + 1];      // only degrees <= PolyDeg<T> are read
@@ -238,6 +241,13 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
             pcnt2 = __ldg(&sg.bin_start[(min(hi - a.n, a.n) - 1) / kBinCells + 1]);
     }
     const int total = pcnt0 + pcnt1 + pcnt2;
+    if (a.skip_empty) {                              // the own FFT's first pass never loads unflagged tiles
+        if (total == 0) return;
+        if (row0 == 0 && threadIdx.x == 0) {
+            const int row = tile >> a.coltile_shift, ct = tile & (a.ncoltiles - 1);
+            atomicOr(&a.row_masks[(si * a.ncoltiles + ct) * 16 + (row & 15)], 1u << (row >> 4));
+        }
+    }
 
     T2 acc[NS][CPT];
 #pragma unroll
@@ -380,6 +390,11 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.tile_stride = p->tile_stride;
     a.tile_mask = (p->ntiles & (p->ntiles - 1)) == 0 ? p->ntiles - 1 : -1;
     a.half = p->poly.half;
+    a.skip_empty = p->own_fft ? 1 : 0;
+    a.row_masks = p->row_masks;
+    a.ncoltiles = (int)std::max<int64_t>(1, p->n / 256 / p->L);
+    a.coltile_shift = 0;
+    while ((1 << a.coltile_shift) < a.ncoltiles) ++a.coltile_shift;
     a.Nd = p->Nd;
     for (int i = 0; i < kHalfMax; ++i)
         for (int d = 0; d <= kMaxDeg; ++d) a.c[i][d] = (T)p->poly.c[i][d];

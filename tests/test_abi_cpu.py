@@ -45,7 +45,8 @@ def test_ls_opts_layout_matches_header():
     assert ls_opts.batch_chunk.offset == 32
     assert ls_opts.no_autotune.offset == 36
     assert ls_opts.graph.offset == 40
-    assert ls_opts.reserved.offset == 44
+    assert ls_opts.fft_impl.offset == 44
+    assert ls_opts.reserved.offset == 48
     assert ctypes.sizeof(ls_opts) == 72
 
 

@@ -65,6 +65,37 @@ def test_cfg3_headline_size_sampled_frequencies():
     assert lo + int(np.argmax(Pg[0][lo:hi])) == kpk
 
 
+def test_cfg3_own_fft_against_cufft_full_grid():
+    """The library's own three-pass FFT (pruned first pass, compact mode output; ls_fft.cu) against the cuFFT
+    path on the FULL grid of the headline config, and both against the oracle's direct sums on sampled k."""
+    import oracle
+    w = make_workload(3)
+    ks = compare_indices(w, 256)
+    P_own, ex_own = gpu_power(w, fft_impl=2, return_plan_info=True, debug_modes=(0, ks))
+    P_cu, ex_cu = gpu_power(w, fft_impl=1, return_plan_info=True, debug_modes=(0, ks))
+    assert ex_own["info"]["n"] == ex_cu["info"]["n"] == 1 << 24
+    assert ex_own["launches"][1] == 0 and ex_cu["launches"][1] == 1      # cuFFT execs per execute
+    assert np.max(np.abs(P_own - P_cu)) / P_cu.max() <= 1e-11            # same spreading, two FFTs
+    _, sums, _ = oracle.direct(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, k=ks, return_sums=True)
+    for g in (ex_own["modes"], ex_cu["modes"]):
+        for a, b in ((0, 1), (2, 3), (4, 5)):
+            num = np.sqrt(np.sum((g[:, a] - sums[:, a]) ** 2 + (g[:, b] - sums[:, b]) ** 2))
+            den = np.sqrt(np.sum(sums[:, a] ** 2 + sums[:, b] ** 2))
+            assert num / den <= w.eps, (a, num / den)
+
+
+def test_own_fft_rejected_where_unsupported():
+    from gpu_util import require_cuda
+    require_cuda()
+    from paper_2409_08090_b200 import binding as B
+    with pytest.raises(B.LsError) as ei:
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=2)     # n = 2^14
+    assert ei.value.code == 5
+    with pytest.raises(B.LsError) as ei:
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=3)
+    assert ei.value.code == 1
+
+
 def test_cfg3_time_shift_invariance_full_grid():
     """A property that holds at any size (north_star: invariance of power to shifting t), on the FULL
     grid of the headline config: P(t + Delta) == P(t) up to the perturbation rounding t + Delta makes."""
