@@ -560,10 +560,12 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
 
             stage_begin(p, LS_STAGE_FFT, s);
             if (p->own_fft) {
-                // own three-pass FFT: pass 1 skips the tiles spreading flagged empty, pass 3 emits the kept modes
+                // own three-pass FFT: pass 1 skips the tiles spreading left unwritten; pass 3 emits compact modes
+                // (shared dy: only of w2, w — the h transforms' pass 3 is fused with the assembly below)
                 const int n_x2 = per ? ps.C : (ps.s0 == 0 ? 1 : 0);
-                LS_TRY(lsb::launch_own_fft(p, ps.fft_slot0, ps.fft_batch, n_x2, true, s));
-                own += 3;
+                const int n_modes = per ? ps.fft_batch : (ps.s0 == 0 ? 2 : 0);
+                LS_TRY(lsb::launch_own_fft(p, ps.fft_slot0, ps.fft_batch, n_x2, n_modes, s));
+                own += n_modes > 0 ? 3 : 2;
             } else {
                 cufftHandle h = find_fft(p, ps.fft_batch);
                 if (cufftSetStream(h, s) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
@@ -578,7 +580,10 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
             stage_end(p, s);
 
             stage_begin(p, LS_STAGE_ASSEMBLE, s);
-            LS_TRY(lsb::launch_assemble(p, ps.s0, ps.C, h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride, power, s));
+            if (p->own_fft && !per)
+                LS_TRY(lsb::launch_own_fft_assemble(p, h_slot, ps.C, ps.s0, w_slot, w2_slot, power, s));
+            else
+                LS_TRY(lsb::launch_assemble(p, ps.s0, ps.C, h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride, power, s));
             ++own;
             stage_end(p, s);
         }
@@ -720,6 +725,7 @@ int ls_debug_modes(ls_plan_t p, int series, int64_t K, const int64_t* kidx, doub
     int rc = LS_OK;
     if (cudaMalloc((void**)&dk, K * 8) != cudaSuccess || cudaMalloc((void**)&dout, K * 48) != cudaSuccess) rc = LS_ERR_ALLOC;
     if (rc == LS_OK && (cudaDeviceSynchronize() != cudaSuccess ||
+                        (p->own_fft && !per && lsb::launch_own_fft_modes(p, h_slot, 0) != cudaSuccess) ||
                         cudaMemcpy(dk, kidx, K * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
                         lsb::launch_debug_modes(p, h_slot, w_slot, w2_slot, K, dk, dout, 0) != cudaSuccess ||
                         cudaMemcpy(out, dout, K * 48, cudaMemcpyDeviceToHost) != cudaSuccess))

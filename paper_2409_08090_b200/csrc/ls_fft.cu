@@ -20,6 +20,7 @@
 // 256-byte global segments on both sides.  Twiddles: w_256 from a shared table, w_n^e from two
 // 4096-entry tables (e = 4096 e_hi + e_lo) and a base/step recurrence along the thread's 16 outputs.
 #include "ls_internal.h"
+#include "ls_power.cuh"
 
 namespace lsb {
 namespace {
@@ -81,6 +82,14 @@ struct FftArgs {
     // pass 3 output
     double2* modes;            // [ntrans][Nf]
     long long Nf, half;
+    // pass 3 fused with deconvolution + assembly (K5 + K6): transform i of the launch is h of series
+    // series0 + i; the (w, w2) modes are read from the compact array
+    const double2* w_modes;    // [Nf] modes of w at x1
+    const double2* w2_modes;   // [Nf] modes of w at x2
+    const double* dinv;        // 1 / psihat(|k'|)
+    const double* sums;        // [batch][4]: YY at [4 s + 2]
+    double* power;             // [batch][Nf]
+    int series0;
 };
 
 __device__ __forceinline__ double2 twiddle_n(const FftArgs& a, unsigned e) {
@@ -196,6 +205,7 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
 // Pass 3: the transform dimension (l3) is contiguous; the CTA takes 16 consecutive k1 at one k2, so that the
 // kept modes leave in runs of 16 consecutive frequencies.  Output: modes[tr][k], k = (kk + half) mod n < Nf,
 // kk = k1 + R1 k2 + R1 R2 k3 the stored mode index (= k' mod n).
+template <bool FUSED>
 __global__ void __launch_bounds__(kFftThreads, 2)
 ls_fft_rows_kernel(const FftArgs a) {
     extern __shared__ __align__(16) unsigned char fsm[];
@@ -224,11 +234,45 @@ ls_fft_rows_kernel(const FftArgs a) {
         double2* out = a.modes + (long long)tr * a.Nf;
         const long long kk0 = (long long)(k1b + c) + (long long)a.R1 * k2;
         const long long r12 = (long long)a.R1 * a.R2;
+        const int ser = a.series0 + tr;
+        const double inv_YY = FUSED ? 1.0 / a.sums[4 * ser + 2] : 0.0;
+        if (FUSED) {
+            // K5: diagonal rescaling of the three modes of frequency k; K6: tau rotation and power.  Four
+            // frequencies at a time: their 12 loads are in flight together before any arithmetic starts.
 #pragma unroll
-        for (int kb = 0; kb < 16; ++kb) {
-            long long k = kk0 + r12 * (ka + 16 * kb) + a.half;
-            if (k >= a.n) k -= a.n;
-            if (k < a.Nf) out[k] = x[pos16(kb)];
+            for (int g = 0; g < 16; g += 4) {
+                long long k[4];
+                double d[4];
+                double2 gw[4], g2[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    k[q] = kk0 + r12 * (ka + 16 * (g + q)) + a.half;
+                    if (k[q] >= a.n) k[q] -= a.n;
+                    d[q] = 0.0;
+                    gw[q] = g2[q] = make_double2(0.0, 0.0);
+                    if (k[q] < a.Nf) {
+                        const long long kp = k[q] - a.half;
+                        d[q] = __ldg(&a.dinv[kp < 0 ? -kp : kp]);
+                        gw[q] = __ldg(&a.w_modes[k[q]]);
+                        g2[q] = __ldg(&a.w2_modes[k[q]]);
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    if (k[q] < a.Nf) {
+                        const double2 gh = x[pos16(g + q)];
+                        const FreqTerms f = freq_terms(gw[q].y * d[q], gw[q].x * d[q], g2[q].y * d[q], g2[q].x * d[q]);
+                        a.power[(long long)ser * a.Nf + k[q]] = series_power(f, gh.y * d[q], gh.x * d[q], inv_YY);
+                    }
+                }
+            }
+        } else {
+#pragma unroll
+            for (int kb = 0; kb < 16; ++kb) {
+                long long k = kk0 + r12 * (ka + 16 * kb) + a.half;
+                if (k >= a.n) k -= a.n;
+                if (k < a.Nf) out[k] = x[pos16(kb)];
+            }
         }
     }
 }
@@ -261,13 +305,11 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if (e != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
-    return cudaFuncSetAttribute(ls_fft_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem);
+    if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
+    return cudaFuncSetAttribute(ls_fft_rows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem);
 }
 
-// FFT of transforms [slot0, slot0 + ntrans) of the plan's grids; the first n_x2 of them belong to the x2
-// point set (pruning flags).  Kept modes land in p->modes[slot0 + i][0..Nf).
-cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, bool prune, cudaStream_t s) {
-    FftArgs a;
+static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.grids = (double2*)p->grids + (long long)slot0 * p->n;
     a.n = p->n;
     a.R1 = a.R2 = a.R3 = 256;
@@ -281,16 +323,52 @@ cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, bool p
     a.modes = (double2*)p->modes + (long long)slot0 * p->Nf;
     a.Nf = p->Nf;
     a.half = p->Nf / 2;
+    a.w_modes = a.w2_modes = nullptr;
+    a.dinv = p->dinv;
+    a.sums = p->sums;
+    a.power = nullptr;
+    a.series0 = 0;
+}
+
+// Passes 1 and 2 of transforms [slot0, slot0 + ntrans) of the plan's grids (the first n_x2 of them belong to
+// the x2 point set: pruning masks), and pass 3 -> compact modes for the first n_modes of them.
+cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, int n_modes, cudaStream_t s) {
+    FftArgs a;
+    fill_common(p, a, slot0, n_x2);
     const long long inner1 = p->n / 256, inner2 = p->n / 65536;
-    dim3 g1((unsigned)(inner1 / 16), 1, ntrans), g2((unsigned)(inner2 / 16), 256, ntrans), g3(256 / 16, 256, ntrans);
-    if (prune) {
-        const int tiles_per_trans = (int)(inner1 / 16), total = tiles_per_trans * ntrans;
-        ls_fft_pass1_kernel<<<std::min(total, 2 * p->num_sms), kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total);
-    } else {
-        ls_fft_cols_kernel<<<g1, kFftThreads, kColsSmem, s>>>(a, 1, inner1);
-    }
+    const int tiles_per_trans = (int)(inner1 / 16), total = tiles_per_trans * ntrans;
+    ls_fft_pass1_kernel<<<std::min(total, 2 * p->num_sms), kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total);
+    dim3 g2((unsigned)(inner2 / 16), 256, ntrans);
     ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, 256, inner2);
-    ls_fft_rows_kernel<<<g3, kFftThreads, kRowsSmem, s>>>(a);
+    if (n_modes > 0) {
+        dim3 g3(256 / 16, 256, n_modes);
+        ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
+    }
+    return cudaGetLastError();
+}
+
+// Pass 3 of the h transforms in slots [h_slot0, h_slot0 + nseries), fused with K5 + K6: power of series
+// series0 + i from its h modes (registers) and the compact (w, w2) modes in slots w_slot, w2_slot.
+cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int series0, int w_slot, int w2_slot,
+                                    void* power, cudaStream_t s) {
+    FftArgs a;
+    fill_common(p, a, h_slot0, 0);
+    a.w_modes = (const double2*)p->modes + (long long)w_slot * p->Nf;
+    a.w2_modes = (const double2*)p->modes + (long long)w2_slot * p->Nf;
+    a.power = (double*)power;
+    a.series0 = series0;
+    dim3 g3(256 / 16, 256, nseries);
+    ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
+    return cudaGetLastError();
+}
+
+// Test hook support: materialise the compact modes of one transform whose pass 3 ran fused (its grid
+// still holds the pass-2 result, which the fused pass only read).
+cudaError_t launch_own_fft_modes(ls_plan_s* p, int slot, cudaStream_t s) {
+    FftArgs a;
+    fill_common(p, a, slot, 0);
+    dim3 g3(256 / 16, 256, 1);
+    ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
 

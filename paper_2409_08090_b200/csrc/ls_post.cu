@@ -7,6 +7,7 @@
 // (Eq. 2; readings A2, A4), stored by the FFT at index k' mod n.  Re g = C, Im g = S
 // (A7).  The assembly runs in fp64 registers for both dtypes (A9).
 #include "ls_internal.h"
+#include "ls_power.cuh"
 
 namespace lsb {
 namespace {
@@ -53,46 +54,6 @@ struct AssembleArgs {
     int h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride;
     void* power;
 };
-
-// The assembly formulas exactly as north_star lists them, with
-//   C2w = |den|/r, S2w = num sign(den)/r, r = hypot(num, den)   [= 1/sqrt(1+tan^2), tan C2w]
-//   Sw  = S2w / (2 Cw)                                           [= sign(S2w) sqrt((1-C2w)/2)]
-// and the conventions of reading A14 for 0/0 and non-positive CC, SS.
-// Per-frequency part (depends on the weights only: shared by every series of a batch with common dy):
-// the rotation (Cw, Sw) = (cos, sin)(omega tau) and the reciprocals of CC, SS (0 where the term is dropped).
-struct FreqTerms {
-    double Cw, Sw, iCC, iSS;
-};
-__device__ __forceinline__ FreqTerms freq_terms(double S, double C, double S2, double C2) {
-    const double num = S2 - 2.0 * S * C;
-    const double den = C2 - (C * C - S * S);
-    const double r = sqrt(num * num + den * den);
-    double C2w = 1.0, S2w = 0.0;
-    if (r > 0.0) {
-        const double ir = 1.0 / r;
-        C2w = fabs(den) * ir;
-        S2w = (den < 0.0 ? -num : num) * ir;
-    }
-    FreqTerms f;
-    f.Cw = sqrt(0.5 * (1.0 + C2w));
-    f.Sw = S2w / (2.0 * f.Cw);
-    const double a = C * f.Cw + S * f.Sw, b = S * f.Cw - C * f.Sw;
-    const double CC = 0.5 * (1.0 + C2 * C2w + S2 * S2w) - a * a;
-    const double SS = 0.5 * (1.0 - C2 * C2w - S2 * S2w) - b * b;
-    f.iCC = CC > 0.0 ? 1.0 / CC : 0.0;
-    f.iSS = SS > 0.0 ? 1.0 / SS : 0.0;
-    return f;
-}
-// Per-series part: YC, YS in the rotated frame and the standard-normalised power.
-__device__ __forceinline__ double series_power(const FreqTerms& f, double Sh, double Ch, double inv_YY) {
-    const double YC = Ch * f.Cw + Sh * f.Sw;
-    const double YS = Sh * f.Cw - Ch * f.Sw;
-    return (YC * YC * f.iCC + YS * YS * f.iSS) * inv_YY;
-}
-__device__ __forceinline__ double assemble_power(double Sh, double Ch, double S, double C, double S2, double C2,
-                                                 double inv_YY) {
-    return series_power(freq_terms(S, C, S2, C2), Sh, Ch, inv_YY);
-}
 
 template <typename T>
 __global__ void __launch_bounds__(kPostThreads)
