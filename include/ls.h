@@ -64,8 +64,11 @@ enum {
     LS_STAGE_SORT = 1,          /* K3  bin count + scan (both point sets)                        */
     LS_STAGE_PREMUL = 2,        /* K2  time-rescale, phase premultiply, scatter to bin order, YY */
     LS_STAGE_SPREAD = 3,        /* K4  tile-owner spreading of all M grids                       */
-    LS_STAGE_FFT = 4,           /* F   cuFFT (library; reported separately, north_star)          */
-    LS_STAGE_ASSEMBLE = 5,      /* K5+K6 mode extraction, deconvolution, tau + power assembly    */
+    LS_STAGE_FFT = 4,           /* F   the fine-grid FFT: cuFFT, or the own passes 1-3 (reported
+                                       separately, north_star)                                   */
+    LS_STAGE_ASSEMBLE = 5,      /* K5+K6 mode extraction, deconvolution, tau + power assembly; with
+                                       the own FFT (fft_impl 0/2) it contains the h transforms'
+                                       third FFT pass, which is fused with it                    */
     LS_STAGE_TOTAL = 6,         /* whole execute                                                 */
     LS_NUM_STAGES = 7
 };
@@ -83,7 +86,8 @@ typedef struct {
     int graph;              /* 0 = auto: small problems replay a captured CUDA graph when timing == 0;
                                1 = never, 2 = always (when timing == 0)                            */
     int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs a
-                               2^24-cell fp64 grid; LS_ERR_UNSUPPORTED otherwise)                   */
+                               2^24-cell fp64 grid; LS_ERR_UNSUPPORTED otherwise), 3 = as 2 but with
+                               deconvolution + assembly as a separate kernel (clean stage timings)  */
     int reserved[5];        /* must be zero                                                       */
 } ls_opts;
 

@@ -337,7 +337,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
                               o.tile_cells > lsb::kSpreadThreads * 4))
         return LS_ERR_INVALID_VALUE;
-    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 2) return LS_ERR_INVALID_VALUE;
+    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 3) return LS_ERR_INVALID_VALUE;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || o.device < 0 || o.device >= ndev) return LS_ERR_CUDA;
@@ -411,7 +411,8 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     p->slots = per ? 3 * p->chunk : 2 + p->chunk;
 
     p->own_fft = o.fft_impl != 1 && lsb::own_fft_supported(p);
-    if (o.fft_impl == 2 && !p->own_fft) { delete p; return LS_ERR_UNSUPPORTED; }
+    if (o.fft_impl >= 2 && !p->own_fft) { delete p; return LS_ERR_UNSUPPORTED; }
+    p->fuse_assemble = p->own_fft && o.fft_impl != 3 && !o.dy_per_series;
 
     // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
     p->ndf = two_prod((double)p->n, df);
@@ -563,7 +564,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 // own three-pass FFT: pass 1 skips the tiles spreading left unwritten; pass 3 emits compact modes
                 // (shared dy: only of w2, w — the h transforms' pass 3 is fused with the assembly below)
                 const int n_x2 = per ? ps.C : (ps.s0 == 0 ? 1 : 0);
-                const int n_modes = per ? ps.fft_batch : (ps.s0 == 0 ? 2 : 0);
+                const int n_modes = !p->fuse_assemble ? ps.fft_batch : (ps.s0 == 0 ? 2 : 0);
                 LS_TRY(lsb::launch_own_fft(p, ps.fft_slot0, ps.fft_batch, n_x2, n_modes, s));
                 own += n_modes > 0 ? 3 : 2;
             } else {
@@ -580,7 +581,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
             stage_end(p, s);
 
             stage_begin(p, LS_STAGE_ASSEMBLE, s);
-            if (p->own_fft && !per)
+            if (p->fuse_assemble)
                 LS_TRY(lsb::launch_own_fft_assemble(p, h_slot, ps.C, ps.s0, w_slot, w2_slot, power, s));
             else
                 LS_TRY(lsb::launch_assemble(p, ps.s0, ps.C, h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride, power, s));
@@ -725,7 +726,7 @@ int ls_debug_modes(ls_plan_t p, int series, int64_t K, const int64_t* kidx, doub
     int rc = LS_OK;
     if (cudaMalloc((void**)&dk, K * 8) != cudaSuccess || cudaMalloc((void**)&dout, K * 48) != cudaSuccess) rc = LS_ERR_ALLOC;
     if (rc == LS_OK && (cudaDeviceSynchronize() != cudaSuccess ||
-                        (p->own_fft && !per && lsb::launch_own_fft_modes(p, h_slot, 0) != cudaSuccess) ||
+                        (p->fuse_assemble && lsb::launch_own_fft_modes(p, h_slot, 0) != cudaSuccess) ||
                         cudaMemcpy(dk, kidx, K * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
                         lsb::launch_debug_modes(p, h_slot, w_slot, w2_slot, K, dk, dout, 0) != cudaSuccess ||
                         cudaMemcpy(out, dout, K * 48, cudaMemcpyDeviceToHost) != cudaSuccess))

@@ -25,7 +25,8 @@
 namespace lsb {
 namespace {
 
-constexpr int kFftThreads = 256;
+constexpr int kC = 16;                   // columns (passes 1, 2) / rows (pass 3) of a CTA's tile
+constexpr int kFftThreads = 16 * kC;
 constexpr double kC1 = 0.92387953251128675613;   // cos(pi/8)
 constexpr double kS1 = 0.38268343236508977173;   // sin(pi/8)
 constexpr double kR2 = 0.70710678118654752440;   // sqrt(1/2)
@@ -98,23 +99,25 @@ __device__ __forceinline__ double2 twiddle_n(const FftArgs& a, unsigned e) {
     return cmul(lo, hi);
 }
 
-// w_256^m table in shared memory, one entry per thread
+// w_256^m table in shared memory
 __device__ __forceinline__ void fill_w256(double2* w256) {
-    double s, c;
-    sincospi((double)threadIdx.x / 128.0, &s, &c);
-    w256[threadIdx.x] = make_double2(c, s);
+    for (int i = threadIdx.x; i < 256; i += kFftThreads) {
+        double s, c;
+        sincospi((double)i / 128.0, &s, &c);
+        w256[i] = make_double2(c, s);
+    }
 }
 
 // Passes 1 and 2: the transform dimension is strided (stride = inner), 16 consecutive columns per CTA.
 // Data viewed as [outer][256][inner]; in place.  Inter-pass twiddle w_n^{k_r * m * outer}.
-__global__ void __launch_bounds__(kFftThreads, 2)
+__global__ void __launch_bounds__(kFftThreads, 512 / kFftThreads)
 ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
-    double2* w256 = Y + 256 * 16;
+    double2* w256 = Y + 256 * kC;
     fill_w256(w256);
-    const int c = threadIdx.x & 15, hi4 = threadIdx.x >> 4;
-    const long long m = (long long)blockIdx.x * 16 + c;      // column
+    const int c = threadIdx.x % kC, hi4 = threadIdx.x / kC;
+    const long long m = (long long)blockIdx.x * kC + c;      // column
     const int o = blockIdx.y, tr = blockIdx.z;
     double2* base = a.grids + (long long)tr * a.n + (long long)o * 256 * inner + m;
 
@@ -126,13 +129,13 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
         fft16(x);
         __syncthreads();                                     // w256 ready
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * 16 + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
     }
     __syncthreads();
     {
         const int ka = hi4;
 #pragma unroll
-        for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * 16 + c];
+        for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * kC + c];
         fft16(x);
         // k_r = ka + 16 kb;  twiddle exponent e = k_r * m * outer (mod n) = e0 + kb * de
         const unsigned mm = (unsigned)m * (unsigned)outer;
@@ -149,17 +152,17 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
 // Pass 1, pruned and persistent: outer = 1, inner = n / 256.  Each CTA walks column tiles (16 columns x 256
 // rows of one transform); the 16-bit liveness mask of the NEXT tile is fetched while the current one is in
 // flight, so the mask never sits on the critical path.  Dead rows are not loaded (they were never written).
-__global__ void __launch_bounds__(kFftThreads, 2)
+__global__ void __launch_bounds__(kFftThreads, 512 / kFftThreads)
 ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int ntiles_total) {
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
-    double2* w256 = Y + 256 * 16;
+    double2* w256 = Y + 256 * kC;
     fill_w256(w256);
-    const int c = threadIdx.x & 15, hi4 = threadIdx.x >> 4;
+    const int c = threadIdx.x % kC, hi4 = threadIdx.x / kC;
     auto mask_of = [&](int tile) -> unsigned {
         if (tile >= ntiles_total) return 0u;
         const int tr = tile / tiles_per_trans;
-        const long long m0 = (long long)(tile - tr * tiles_per_trans) * 16;
+        const long long m0 = (long long)(tile - tr * tiles_per_trans) * kC;
         const int set = tr < a.set_of_trans_first ? 0 : 1;
         return __ldg(&a.row_masks[((long long)set * a.ncoltiles + (m0 >> a.tile_shift)) * 16 + hi4]);
     };
@@ -168,7 +171,7 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
     __syncthreads();                                         // w256 ready
     for (; tile < ntiles_total; tile += gridDim.x) {
         const int tr = tile / tiles_per_trans;
-        const long long m = (long long)(tile - tr * tiles_per_trans) * 16 + c;
+        const long long m = (long long)(tile - tr * tiles_per_trans) * kC + c;
         double2* base = a.grids + (long long)tr * a.n + m;
         double2 x[16];
         {
@@ -181,13 +184,13 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
             live = mask_of(tile + gridDim.x);                // prefetch: lands during this tile's work
             fft16(x);
 #pragma unroll
-            for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * 16 + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+            for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
         }
         __syncthreads();
         {
             const int ka = hi4;
 #pragma unroll
-            for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * 16 + c];
+            for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * kC + c];
             fft16(x);
             const unsigned mm = (unsigned)m;
             double2 tw = twiddle_n(a, (unsigned)ka * mm);
@@ -206,13 +209,13 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
 // kept modes leave in runs of 16 consecutive frequencies.  Output: modes[tr][k], k = (kk + half) mod n < Nf,
 // kk = k1 + R1 k2 + R1 R2 k3 the stored mode index (= k' mod n).
 template <bool FUSED>
-__global__ void __launch_bounds__(kFftThreads, 2)
+__global__ void __launch_bounds__(kFftThreads, 512 / kFftThreads)
 ls_fft_rows_kernel(const FftArgs a) {
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][17] (padded: conflict-free both ways)
-    double2* w256 = Y + 256 * 17;
+    double2* w256 = Y + 256 * (kC + 1);
     fill_w256(w256);
-    const int k1b = blockIdx.x * 16, k2 = blockIdx.y, tr = blockIdx.z;
+    const int k1b = blockIdx.x * kC, k2 = blockIdx.y, tr = blockIdx.z;
     const double2* src = a.grids + (long long)tr * a.n;
     double2 x[16];
     {
@@ -223,13 +226,13 @@ ls_fft_rows_kernel(const FftArgs a) {
         fft16(x);
         __syncthreads();
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * 17 + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (kC + 1) + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
     }
     __syncthreads();
     {
-        const int c = threadIdx.x & 15, ka = threadIdx.x >> 4;
+        const int c = threadIdx.x % kC, ka = threadIdx.x / kC;
 #pragma unroll
-        for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * 17 + c];
+        for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * (kC + 1) + c];
         fft16(x);
         double2* out = a.modes + (long long)tr * a.Nf;
         const long long kk0 = (long long)(k1b + c) + (long long)a.R1 * k2;
@@ -291,8 +294,8 @@ __global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
     }
 }
 
-constexpr size_t kColsSmem = sizeof(double2) * (256 * 16 + 256);
-constexpr size_t kRowsSmem = sizeof(double2) * (256 * 17 + 256);
+constexpr size_t kColsSmem = sizeof(double2) * (256 * kC + 256);
+constexpr size_t kRowsSmem = sizeof(double2) * (256 * (kC + 1) + 256);
 
 }  // namespace
 
@@ -336,12 +339,12 @@ cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, int n_
     FftArgs a;
     fill_common(p, a, slot0, n_x2);
     const long long inner1 = p->n / 256, inner2 = p->n / 65536;
-    const int tiles_per_trans = (int)(inner1 / 16), total = tiles_per_trans * ntrans;
-    ls_fft_pass1_kernel<<<std::min(total, 2 * p->num_sms), kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total);
-    dim3 g2((unsigned)(inner2 / 16), 256, ntrans);
+    const int tiles_per_trans = (int)(inner1 / kC), total = tiles_per_trans * ntrans;
+    ls_fft_pass1_kernel<<<std::min(total, (512 / kFftThreads) * p->num_sms), kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total);
+    dim3 g2((unsigned)(inner2 / kC), 256, ntrans);
     ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, 256, inner2);
     if (n_modes > 0) {
-        dim3 g3(256 / 16, 256, n_modes);
+        dim3 g3(256 / kC, 256, n_modes);
         ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     }
     return cudaGetLastError();
@@ -357,7 +360,7 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
     a.w2_modes = (const double2*)p->modes + (long long)w2_slot * p->Nf;
     a.power = (double*)power;
     a.series0 = series0;
-    dim3 g3(256 / 16, 256, nseries);
+    dim3 g3(256 / kC, 256, nseries);
     ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
@@ -367,7 +370,7 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
 cudaError_t launch_own_fft_modes(ls_plan_s* p, int slot, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot, 0);
-    dim3 g3(256 / 16, 256, 1);
+    dim3 g3(256 / kC, 256, 1);
     ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }

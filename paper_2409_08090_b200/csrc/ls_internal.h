@@ -108,6 +108,7 @@ struct ls_plan_s {
     size_t total_bytes = 0;
     // own FFT (ls_fft.cu): n = 2^24 fp64; opts.fft_impl
     bool own_fft = false;
+    bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
     void* modes = nullptr;                          // [slots][Nf] complex: kept modes in frequency order
     unsigned* row_masks = nullptr;                  // [2][n/256/L][16] liveness bits for FFT pass 1 (in `zeroed`)

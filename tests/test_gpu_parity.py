@@ -76,6 +76,7 @@ def test_cfg3_own_fft_against_cufft_full_grid():
     assert ex_own["info"]["n"] == ex_cu["info"]["n"] == 1 << 24
     assert ex_own["launches"][1] == 0 and ex_cu["launches"][1] == 1      # cuFFT execs per execute
     assert np.max(np.abs(P_own - P_cu)) / P_cu.max() <= 1e-11            # same spreading, two FFTs
+    assert np.max(np.abs(gpu_power(w, fft_impl=3) - P_own)) <= 1e-13     # unfused assembly: same arithmetic
     _, sums, _ = oracle.direct(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, k=ks, return_sums=True)
     for g in (ex_own["modes"], ex_cu["modes"]):
         for a, b in ((0, 1), (2, 3), (4, 5)):
@@ -92,7 +93,7 @@ def test_own_fft_rejected_where_unsupported():
         B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=2)     # n = 2^14
     assert ei.value.code == 5
     with pytest.raises(B.LsError) as ei:
-        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=3)
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=4)
     assert ei.value.code == 1
 
 
