@@ -209,28 +209,50 @@ def whole_job_value(total_ms, steps, batch, world):
 STAGE_BYTES_DOC = "DESIGN.md §6"
 
 
-def stage_model_bytes(w, info):
-    """Algorithmic HBM bytes per execute of each own stage: every
-    intermediate written once and read once, nothing counted for re-reads or halo candidates."""
+def occupied_tile_rows(w, info, L):
+    """(tiles holding points) x (transforms of that point set), summed over the two point sets — what the
+    spreading kernel writes and the first FFT pass reads when the own FFT is used (empty tiles are never
+    written).  Host-side count from the inputs; plain doubles are ample for counting tiles."""
+    n, wd = info["n"], info["w"]
+    ntiles = (n + L - 1) // L
+    u1 = np.mod(n * w.df * w.t, n)
+    out = 0
+    for u, rows in ((u1, 1 + w.batch), (np.mod(2.0 * u1, n), 1)):
+        lo = np.floor((u - wd / 2 - 1) / L).astype(np.int64) % ntiles
+        hi = np.floor((u + wd / 2 + 1) / L).astype(np.int64) % ntiles
+        out += np.union1d(lo, hi).size * rows
+    return out
+
+
+def stage_model_bytes(w, info, own_fft, L):
+    """Algorithmic HBM bytes per execute of each own kernel: every
+    intermediate written once and read once, nothing counted for re-reads or halo candidates.  With the
+    own FFT the fine grids are sparse (only tiles that hold points exist), so the grid term of the
+    spreading kernel and of the first FFT pass's reads is the occupied part, not M n."""
     B = 8 if w.dtype == "f64" else 4
     Nd, Nf, n, M, batch = w.Nd, w.Nf, info["n"], info["M"], w.batch
     nbins = n // 64
     rec = 4 * B                                           # one bin-sorted point record (32 B fp64 / 16 B fp32)
     rows = M * Nd * B                                     # real strengths, one row per transform
-    return {
+    grid = M * n * 2 * B
+    written = occupied_tile_rows(w, info, L) * L * 2 * B if own_fft else grid
+    d = {
         "stats": 8 * Nd + batch * Nd * B + Nd * B + 2 * 4 * nbins,
         "sort": 3 * 2 * 4 * nbins,
         "premul": 8 * Nd + batch * Nd * B + Nd * B + 2 * Nd * rec + rows + (0 if batch == 1 else 2 * 4 * Nd),
-        "spread": M * n * 2 * B + 2 * Nd * rec + rows,
+        "spread": written + 2 * Nd * rec + rows,
         "assemble": M * Nf * 2 * B + batch * Nf * B + (Nf // 2 + 1) * 8,
     }
+    if own_fft:
+        d.update({"fft_pass1": written + grid, "fft_pass2": 2 * grid, "fft_pass3": grid + M * Nf * 2 * B})
+    return d
 
 
 def measured_traffic(kernel_stage, w, info):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    ncu --set full capture (profiles/r1c_traffic.csv; same command line, config 3 defaults).  None when
+    ncu --set full capture (profiles/r1d_traffic.csv; same command line, config 3 defaults).  None when
     the capture does not cover this workload / plan."""
-    path = os.path.join(ROOT, "profiles", "r1c_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r1d_traffic.csv")
     try:
         with open(path) as f:
             rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
@@ -356,12 +378,15 @@ def run_ours(args):
     ms_per_step, value = whole_job_value(dev_ms, args.steps, w.batch, world)
     stage = {k: v / args.steps for k, v in stage_acc.items()}
     peak, peak_src = measured_peak()
-    sbytes = stage_model_bytes(w, info)
-    own_stages = [k for k in ("stats", "sort", "premul", "spread", "assemble")]
-    dom = max(own_stages, key=lambda k: stage[k])
+    own_fft = ffts == 0
+    L = args.tile_cells or (1024 if w.batch == 1 else 512)
+    sbytes = stage_model_bytes(w, info, own_fft, L)
+    own_stages = ["stats", "sort", "premul", "spread", "assemble"] + (["fft_pass1", "fft_pass2", "fft_pass3"] if own_fft else [])
+    dom = max(own_stages, key=lambda k: stage[k])      # the dominant OWN kernel (cuFFT, when used, is a library)
     ach = sbytes[dom] / (stage[dom] * 1e-3) / 1e9
     path_ms = stage["total"] - stage["fft"]
     path_ach = info["model_bytes"] / (path_ms * 1e-3) / 1e9
+    path_sparse = info["model_bytes"] - (info["M"] * info["n"] * 2 * (8 if w.dtype == "f64" else 4) - (sbytes["spread"] - 2 * w.Nd * 4 * (8 if w.dtype == "f64" else 4) - info["M"] * w.Nd * (8 if w.dtype == "f64" else 4)))
     Bi = ht.numel() * ht.element_size() + hy.numel() * hy.element_size() + hdy.numel() * hdy.element_size()
     Bo = hP.numel() * hP.element_size()
     line = {
@@ -377,9 +402,12 @@ def run_ours(args):
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                      "traffic": measured_traffic(dom, w, info), "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
                      "kernel_ms": stage[dom]},
-        "path_roofline": {"what": "all own kernels (total - cuFFT), model bytes of " + STAGE_BYTES_DOC,
-                          "bytes": info["model_bytes"], "ms": path_ms, "achieved": path_ach, "unit": "GB/s",
-                          "frac_of_measured": path_ach / peak, "frac_of_8TBs": path_ach / 8000.0},
+        "path_roofline": {"what": "spread + deconvolve + assembly path = all own kernels except the FFT (total - fft), "
+                                  "bytes = streaming model of " + STAGE_BYTES_DOC + "; bytes_sparse = the same with the "
+                                  "grid term reduced to the tiles that hold points (what the own-FFT path really writes)",
+                          "bytes": info["model_bytes"], "bytes_sparse": path_sparse, "ms": path_ms, "achieved": path_ach,
+                          "unit": "GB/s", "frac_of_measured": path_ach / peak, "frac_of_8TBs": path_ach / 8000.0,
+                          "achieved_sparse": path_sparse / (path_ms * 1e-3) / 1e9},
         "fft_ms": stage["fft"],
         "fft": {"impl": "cuFFT" if ffts else "own three radix-256 passes (first pruned by the spreading kernel's "
                                              "liveness masks; in `value` the last is fused with the assembly)",

@@ -70,7 +70,10 @@ enum {
                                        the own FFT (fft_impl 0/2) it contains the h transforms'
                                        third FFT pass, which is fused with it                    */
     LS_STAGE_TOTAL = 6,         /* whole execute                                                 */
-    LS_NUM_STAGES = 7
+    LS_STAGE_FFT_PASS1 = 7,     /* own FFT only: the three passes, also summed into LS_STAGE_FFT  */
+    LS_STAGE_FFT_PASS2 = 8,
+    LS_STAGE_FFT_PASS3 = 9,     /*   (pass 3 of the transforms whose modes go to the compact array) */
+    LS_NUM_STAGES = 10
 };
 
 /* Optional tuning; a zero-initialised struct (or NULL) selects the defaults. */

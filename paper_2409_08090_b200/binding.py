@@ -20,7 +20,7 @@ __all__ = [
 
 LS_F32, LS_F64 = 0, 1
 LS_OK = 0
-STAGES = ("stats", "sort", "premul", "spread", "fft", "assemble", "total")
+STAGES = ("stats", "sort", "premul", "spread", "fft", "assemble", "total", "fft_pass1", "fft_pass2", "fft_pass3")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB = os.path.join(_HERE, "libls_b200.so")

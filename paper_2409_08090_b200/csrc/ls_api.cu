@@ -559,15 +559,23 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
             }
             stage_end(p, s);
 
-            stage_begin(p, LS_STAGE_FFT, s);
             if (p->own_fft) {
                 // own three-pass FFT: pass 1 skips the tiles spreading left unwritten; pass 3 emits compact modes
-                // (shared dy: only of w2, w — the h transforms' pass 3 is fused with the assembly below)
+                // (fused mode: only of w2, w — the h transforms' pass 3 is part of the assembly kernel below)
                 const int n_x2 = per ? ps.C : (ps.s0 == 0 ? 1 : 0);
                 const int n_modes = !p->fuse_assemble ? ps.fft_batch : (ps.s0 == 0 ? 2 : 0);
-                LS_TRY(lsb::launch_own_fft(p, ps.fft_slot0, ps.fft_batch, n_x2, n_modes, s));
+                stage_begin(p, LS_STAGE_FFT_PASS1, s);
+                LS_TRY(lsb::launch_own_fft_pass1(p, ps.fft_slot0, ps.fft_batch, n_x2, s));
+                stage_end(p, s);
+                stage_begin(p, LS_STAGE_FFT_PASS2, s);
+                LS_TRY(lsb::launch_own_fft_pass2(p, ps.fft_slot0, ps.fft_batch, s));
+                stage_end(p, s);
+                stage_begin(p, LS_STAGE_FFT_PASS3, s);
+                LS_TRY(lsb::launch_own_fft_pass3(p, ps.fft_slot0, n_modes, s));
+                stage_end(p, s);
                 own += n_modes > 0 ? 3 : 2;
             } else {
+                stage_begin(p, LS_STAGE_FFT, s);
                 cufftHandle h = find_fft(p, ps.fft_batch);
                 if (cufftSetStream(h, s) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
                 char* base = (char*)p->grids + (size_t)ps.fft_slot0 * p->n * 2 * real_bytes(p->dtype);
@@ -577,8 +585,8 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                                      : cufftExecC2C(h, (cufftComplex*)base, (cufftComplex*)base, CUFFT_INVERSE);
                 if (fr != CUFFT_SUCCESS) return LS_ERR_CUFFT;
                 ++ffts;
+                stage_end(p, s);
             }
-            stage_end(p, s);
 
             stage_begin(p, LS_STAGE_ASSEMBLE, s);
             if (p->fuse_assemble)
@@ -680,6 +688,7 @@ int ls_get_stage_ms(ls_plan_t p, float* ms, int n_stages) {
         float v = 0;
         if (cudaEventElapsedTime(&v, ev.beg, ev.end) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
         acc[ev.stage] += v;
+        if (ev.stage >= LS_STAGE_FFT_PASS1 && ev.stage <= LS_STAGE_FFT_PASS3) acc[LS_STAGE_FFT] += v;
     }
     for (int i = 0; i < n_stages && i < LS_NUM_STAGES; ++i) ms[i] = acc[i];
     return LS_OK;
@@ -726,7 +735,7 @@ int ls_debug_modes(ls_plan_t p, int series, int64_t K, const int64_t* kidx, doub
     int rc = LS_OK;
     if (cudaMalloc((void**)&dk, K * 8) != cudaSuccess || cudaMalloc((void**)&dout, K * 48) != cudaSuccess) rc = LS_ERR_ALLOC;
     if (rc == LS_OK && (cudaDeviceSynchronize() != cudaSuccess ||
-                        (p->fuse_assemble && lsb::launch_own_fft_modes(p, h_slot, 0) != cudaSuccess) ||
+                        (p->fuse_assemble && lsb::launch_own_fft_pass3(p, h_slot, 1, 0) != cudaSuccess) ||
                         cudaMemcpy(dk, kidx, K * 8, cudaMemcpyHostToDevice) != cudaSuccess ||
                         lsb::launch_debug_modes(p, h_slot, w_slot, w2_slot, K, dk, dout, 0) != cudaSuccess ||
                         cudaMemcpy(out, dout, K * 48, cudaMemcpyDeviceToHost) != cudaSuccess))

@@ -333,20 +333,34 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.series0 = 0;
 }
 
-// Passes 1 and 2 of transforms [slot0, slot0 + ntrans) of the plan's grids (the first n_x2 of them belong to
-// the x2 point set: pruning masks), and pass 3 -> compact modes for the first n_modes of them.
-cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, int n_modes, cudaStream_t s) {
+// Pass 1 of transforms [slot0, slot0 + ntrans) of the plan's grids; the first n_x2 of them belong to the x2
+// point set (which liveness masks to prune by).
+cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot0, n_x2);
-    const long long inner1 = p->n / 256, inner2 = p->n / 65536;
+    const long long inner1 = p->n / 256;
     const int tiles_per_trans = (int)(inner1 / kC), total = tiles_per_trans * ntrans;
-    ls_fft_pass1_kernel<<<std::min(total, (512 / kFftThreads) * p->num_sms), kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total);
+    ls_fft_pass1_kernel<<<std::min(total, (512 / kFftThreads) * p->num_sms), kFftThreads, kColsSmem, s>>>(
+        a, inner1, tiles_per_trans, total);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
+    FftArgs a;
+    fill_common(p, a, slot0, 0);
+    const long long inner2 = p->n / 65536;
     dim3 g2((unsigned)(inner2 / kC), 256, ntrans);
     ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, 256, inner2);
-    if (n_modes > 0) {
-        dim3 g3(256 / kC, 256, n_modes);
-        ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
-    }
+    return cudaGetLastError();
+}
+
+// Pass 3 -> compact modes, transforms [slot0, slot0 + ntrans).
+cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
+    if (ntrans <= 0) return cudaSuccess;
+    FftArgs a;
+    fill_common(p, a, slot0, 0);
+    dim3 g3(256 / kC, 256, ntrans);
+    ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
 
@@ -362,16 +376,6 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
     a.series0 = series0;
     dim3 g3(256 / kC, 256, nseries);
     ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
-    return cudaGetLastError();
-}
-
-// Test hook support: materialise the compact modes of one transform whose pass 3 ran fused (its grid
-// still holds the pass-2 result, which the fused pass only read).
-cudaError_t launch_own_fft_modes(ls_plan_s* p, int slot, cudaStream_t s) {
-    FftArgs a;
-    fill_common(p, a, slot, 0);
-    dim3 g3(256 / kC, 256, 1);
-    ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
 

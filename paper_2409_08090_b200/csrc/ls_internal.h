@@ -141,8 +141,9 @@ int spread_rows_per_group(const ls_plan_s* p);
 // ---- ls_fft.cu: own three-pass FFT (n = 2^24, fp64) ------------------------------------------
 bool own_fft_supported(const ls_plan_s* p);
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
-cudaError_t launch_own_fft(ls_plan_s* p, int slot0, int ntrans, int n_x2, int n_modes, cudaStream_t s);
-cudaError_t launch_own_fft_modes(ls_plan_s* p, int slot, cudaStream_t s);
+cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s);
+cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
+cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
 cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int series0, int w_slot, int w2_slot,
                                     void* power, cudaStream_t s);
 // ---- ls_post.cu: P0 table, K5+K6 -----------------------------------------------------------
