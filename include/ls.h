@@ -127,8 +127,16 @@ int ls_execute_host(ls_plan_t plan, const void* t, const void* y, const void* dy
 int ls_get_info(ls_plan_t plan, double* sigma, int* w, double* beta, int64_t* n, int* M,
                 double* model_bytes);
 
-/* Device bytes the plan allocated (grids + cuFFT work area + tables + scratch). */
+/* Device bytes the plan allocated (grids + mode array + FFT work area + tables + scratch). */
 size_t ls_workspace_bytes(ls_plan_t plan);
+
+/* ls_set_workspace — run the plan's large buffers (fine grids, compact mode array, cuFFT work area)
+ * inside caller-owned device memory, e.g. a torch allocation: `dptr` must be 256-byte aligned and hold
+ * at least ls_workspace_bytes(plan) bytes (more than the three buffers need, so that size always
+ * suffices).  The plan frees its own copies; the caller keeps ownership of `dptr` and must keep it alive
+ * until ls_destroy or the next ls_set_workspace.  Not to be called while an execute is in flight.
+ * Errors: LS_ERR_INVALID_VALUE (NULL plan or pointer, misaligned, too small), LS_ERR_CUFFT. */
+int ls_set_workspace(ls_plan_t plan, void* dptr, size_t bytes);
 
 /* Milliseconds per stage of the most recent execute (needs opts.timing = 1; synchronises on the
  * recorded events).  ms[LS_NUM_STAGES]; n_stages entries are written.  LS_ERR_NOT_READY if no

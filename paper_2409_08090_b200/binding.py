@@ -13,7 +13,7 @@ import os
 
 __all__ = [
     "LS_F32", "LS_F64", "LS_OK", "STAGES", "LsError", "ls_opts", "lib_path", "load",
-    "ls_plan", "ls_execute", "ls_execute_host", "ls_destroy", "ls_get_info", "ls_workspace_bytes",
+    "ls_plan", "ls_execute", "ls_execute_host", "ls_destroy", "ls_get_info", "ls_workspace_bytes", "ls_set_workspace",
     "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_strerror",
     "exported_symbols", "Plan",
 ]
@@ -59,6 +59,7 @@ _SIGNATURES = {
     "ls_get_info": (C.c_int, [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_int), C.POINTER(C.c_double),
                               C.POINTER(C.c_int64), C.POINTER(C.c_int), C.POINTER(C.c_double)]),
     "ls_workspace_bytes": (C.c_size_t, [C.c_void_p]),
+    "ls_set_workspace": (C.c_int, [C.c_void_p, C.c_void_p, C.c_size_t]),
     "ls_get_stage_ms": (C.c_int, [C.c_void_p, C.POINTER(C.c_float), C.c_int]),
     "ls_get_launch_counts": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "ls_debug_modes": (C.c_int, [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]),
@@ -151,6 +152,12 @@ def ls_workspace_bytes(plan) -> int:
     return int(load().ls_workspace_bytes(plan))
 
 
+def ls_set_workspace(plan, buf, nbytes: int) -> None:
+    rc = load().ls_set_workspace(plan, C.c_void_p(_ptr(buf)), C.c_size_t(int(nbytes)))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_set_workspace")
+
+
 def ls_get_stage_ms(plan) -> dict:
     ms = (C.c_float * len(STAGES))()
     rc = load().ls_get_stage_ms(plan, ms, len(STAGES))
@@ -217,6 +224,11 @@ class Plan:
 
     def workspace_bytes(self):
         return ls_workspace_bytes(self.handle)
+
+    def set_workspace(self, buf, nbytes):
+        """Move the plan's large buffers into caller-owned device memory (keep `buf` alive)."""
+        ls_set_workspace(self.handle, buf, nbytes)
+        self._workspace = buf
 
     def close(self):
         if self.handle:

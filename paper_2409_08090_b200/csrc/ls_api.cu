@@ -293,12 +293,14 @@ int ls_destroy(ls_plan_t p) {
     if (p->has_first) cufftDestroy(p->fft_first);
     if (p->has_chunk) cufftDestroy(p->fft_chunk);
     if (p->has_rem) cufftDestroy(p->fft_rem);
-    cudaFree(p->fft_work);
-    cudaFree(p->grids);
+    if (!p->external_ws) {
+        cudaFree(p->fft_work);
+        cudaFree(p->grids);
+        cudaFree(p->modes);
+    }
     cudaFree(p->dinv);
     cudaFree(p->fft_wlo);
     cudaFree(p->fft_whi);
-    cudaFree(p->modes);
     cudaFree(p->zeroed);                     // sums and both histograms live in this allocation
     cudaFree(p->scan_tmp);
     for (int i = 0; i < 2; ++i) {
@@ -426,12 +428,14 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     int rc = LS_OK;
     cudaError_t ce = cudaSuccess;
     do {
-        if ((ce = dmalloc(p, &p->grids, (size_t)p->slots * grid_bytes)) != cudaSuccess) break;
+        p->grids_bytes = (size_t)p->slots * grid_bytes;
+        if ((ce = dmalloc(p, &p->grids, p->grids_bytes)) != cudaSuccess) break;
         if ((ce = dmalloc(p, &p->dinv, (size_t)(Nf / 2 + 1) * 8)) != cudaSuccess) break;
         if (p->own_fft) {
             if ((ce = dmalloc(p, (char**)&p->fft_wlo, (size_t)4096 * 16)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&p->fft_whi, (size_t)std::max<int64_t>(4096, p->n / 4096) * 16)) != cudaSuccess) break;
-            if ((ce = dmalloc(p, (char**)&p->modes, (size_t)p->slots * Nf * 16)) != cudaSuccess) break;
+            p->modes_bytes = (size_t)p->slots * Nf * 16;
+            if ((ce = dmalloc(p, (char**)&p->modes, p->modes_bytes)) != cudaSuccess) break;
             if ((ce = lsb::own_fft_init(p, 0)) != cudaSuccess) break;
         }
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
@@ -677,6 +681,34 @@ int ls_get_info(ls_plan_t p, double* sigma, int* w, double* beta, int64_t* n, in
 }
 
 size_t ls_workspace_bytes(ls_plan_t p) { return p ? p->total_bytes : 0; }
+
+int ls_set_workspace(ls_plan_t p, void* dptr, size_t bytes) {
+    if (!p || !dptr || ((uintptr_t)dptr & 255) != 0) return LS_ERR_INVALID_VALUE;
+    auto up = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t need = up(p->grids_bytes) + up(p->modes_bytes) + up(p->fft_work_bytes);
+    if (bytes < need || bytes < p->total_bytes) return LS_ERR_INVALID_VALUE;
+    if (cudaSetDevice(p->opts.device) != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    if (!p->external_ws) {
+        cudaFree(p->grids);
+        cudaFree(p->modes);
+        cudaFree(p->fft_work);
+    }
+    char* base = (char*)dptr;
+    p->grids = base;
+    p->modes = p->modes_bytes ? base + up(p->grids_bytes) : nullptr;
+    p->fft_work = base + up(p->grids_bytes) + up(p->modes_bytes);
+    p->external_ws = true;
+    if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }     // captured pointers are stale
+    if (!p->own_fft) {
+        if (cufftSetWorkArea(p->fft_first, p->fft_work) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+        if (p->has_chunk && cufftSetWorkArea(p->fft_chunk, p->fft_work) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+        if (p->has_rem && cufftSetWorkArea(p->fft_rem, p->fft_work) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
+    }
+    return LS_OK;
+}
 
 int ls_get_stage_ms(ls_plan_t p, float* ms, int n_stages) {
     if (!p || !ms || n_stages < 1) return LS_ERR_INVALID_VALUE;

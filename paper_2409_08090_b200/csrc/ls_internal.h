@@ -106,6 +106,8 @@ struct ls_plan_s {
     void* fft_work = nullptr;
     size_t fft_work_bytes = 0;
     size_t total_bytes = 0;
+    size_t grids_bytes = 0, modes_bytes = 0;
+    bool external_ws = false;   // grids / modes / fft_work live in caller memory (ls_set_workspace)
     // own FFT (ls_fft.cu): n = 2^24 fp64; opts.fft_impl
     bool own_fft = false;
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6

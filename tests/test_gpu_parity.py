@@ -216,6 +216,29 @@ def test_per_series_dy():
             _check64(errors(Pg[b], oracle_power(w, b)))
 
 
+def test_caller_owned_workspace():
+    """ls_set_workspace: grids, mode array and FFT work area inside a torch allocation; same results."""
+    import torch
+    from paper_2409_08090_b200 import binding as B
+    w = scaled_workload(2, 3000)
+    P_ref = gpu_power(w)
+    dev = torch.device("cuda:0")
+    t = torch.from_numpy(w.t).to(dev); y = torch.from_numpy(w.y).to(dev); dy = torch.from_numpy(w.dy).to(dev)
+    P = torch.empty((1, w.Nf), dtype=torch.float64, device=dev)
+    with B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F64, 1) as plan:
+        nbytes = plan.workspace_bytes()
+        ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=dev)
+        off = (-ws.data_ptr()) % 256
+        with pytest.raises(B.LsError):
+            plan.set_workspace(ws.data_ptr() + off, nbytes // 2)         # too small
+        with pytest.raises(B.LsError):
+            plan.set_workspace(ws.data_ptr() + off + 8, nbytes)          # misaligned
+        plan.set_workspace(ws.data_ptr() + off, nbytes)
+        plan.execute(t, y, dy, P, torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    assert np.max(np.abs(P.cpu().numpy() - P_ref)) <= 1e-13
+
+
 def test_execute_host_matches_device():
     w = scaled_workload(2, 2500)
     Pd = gpu_power(w)
