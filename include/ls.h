@@ -88,8 +88,8 @@ typedef struct {
     int no_autotune;        /* 1: never time candidate grid sizes at plan time (auto n = power of two) */
     int graph;              /* 0 = auto: small problems replay a captured CUDA graph when timing == 0;
                                1 = never, 2 = always (when timing == 0)                            */
-    int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs a
-                               2^24-cell fp64 grid; LS_ERR_UNSUPPORTED otherwise), 3 = as 2 but with
+    int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs an
+                               fp64 grid of 2^20..2^24 cells; LS_ERR_UNSUPPORTED otherwise), 3 = as 2 but with
                                deconvolution + assembly as a separate kernel (clean stage timings)  */
     int reserved[5];        /* must be zero                                                       */
 } ls_opts;

@@ -441,7 +441,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
-        const size_t mask_bytes = p->own_fft ? (size_t)2 * (p->n / 256 / p->L) * 16 * 4 : 0;
+        const size_t mask_bytes = p->own_fft ? (size_t)2 * (65536 / p->L) * 16 * 4 : 0;
         p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
         if (p->own_fft) p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes);

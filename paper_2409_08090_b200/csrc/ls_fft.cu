@@ -1,9 +1,10 @@
-// ls_fft.cu — the library's own fine-grid FFT for n = 2^24 complex128 grids (
+// ls_fft.cu — the library's own fine-grid FFT for complex128 grids of n = 2^20 .. 2^24 cells (
 // PAPER.md:47 "use an equispaced FFT", :73 "the FFT time dominates").
 //
 //   B_k = sum_l b_l e^{+2 pi i k l / n}     (reading A7: the unnormalised inverse transform)
 //
-// Three radix-256 passes over n = R1 R2 R3 = 256^3, decimation in frequency:
+// Three passes over n = R1 R2 R3, R2 = R3 = 256, R1 = n / 2^16 = 16 .. 256 (256^3 at the headline size),
+// decimation in frequency:
 //   l = l1 R2 R3 + l2 R3 + l3,   k = k1 + R1 k2 + R1 R2 k3
 //   pass 1: FFT over l1 -> k1, times w_n^{k1 (l2 R3 + l3)};   in place, layout [k1][l2][l3]
 //   pass 2: FFT over l2 -> k2, times w_n^{R1 k2 l3};          in place, layout [k1][k2][l3]
@@ -67,15 +68,47 @@ __device__ __forceinline__ void fft16(double2 (&x)[16]) {
     for (int ka = 0; ka < 4; ++ka) fft4(x[4 * ka], x[4 * ka + 1], x[4 * ka + 2], x[4 * ka + 3]);
 }
 
+// 8-point transform (two fft4 on the even / odd samples, then a radix-2 layer); X_k ends at position
+// pos8(k) = 2 (k & 3) + (k >> 2).
+__device__ __forceinline__ void fft8(double2 (&x)[8]) {
+    fft4(x[0], x[2], x[4], x[6]);
+    fft4(x[1], x[3], x[5], x[7]);
+    x[3] = cmul(x[3], make_double2(kR2, kR2));       // w_8^1
+    x[5] = cmuli(x[5]);                              // w_8^2
+    x[7] = cmul(x[7], make_double2(-kR2, kR2));      // w_8^3
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const double2 e = x[2 * k], o = x[2 * k + 1];
+        x[2 * k] = cadd(e, o);
+        x[2 * k + 1] = csub(e, o);
+    }
+}
+// RB-point transform, RB in {1, 2, 4, 8, 16}: in place, X_k at position fft_pos<RB>(k).
+template <int RB>
+__device__ __forceinline__ constexpr int fft_pos(int k) {
+    return RB == 16 ? 4 * (k & 3) + (k >> 2) : RB == 8 ? 2 * (k & 3) + (k >> 2) : k;
+}
+template <int RB>
+__device__ __forceinline__ void fft_small(double2 (&x)[RB]) {
+    if constexpr (RB == 16) fft16(x);
+    else if constexpr (RB == 8) fft8(x);
+    else if constexpr (RB == 4) fft4(x[0], x[1], x[2], x[3]);
+    else if constexpr (RB == 2) {
+        const double2 a = x[0], b = x[1];
+        x[0] = cadd(a, b);
+        x[1] = csub(a, b);
+    }
+}
+
 struct FftArgs {
     double2* grids;            // [ntrans][n] in place
     long long n;
-    int R1, R2, R3;            // 256 each
+    int R1, R2, R3;            // n = R1 * 256 * 256, R1 = 16 RB in {16 .. 256}
     const double2* wlo;        // w_n^x, x < 4096
     const double2* whi;        // w_n^{4096 y}, y < n / 4096
     // pass 1 pruning (see PointSet-independent `row_masks` in ls_internal.h): for point set s, spreading-tile
-    // column ct = (m >> tile_shift) and j = row & 15, bit i of row_masks[(s * ncoltiles + ct) * 16 + j] says
-    // that row 16 i + j of that column holds data; unset = never written by the spreading kernel = zeros.
+    // column ct = (m >> tile_shift) and j = row % RB (RB = R1/16), bit i of row_masks[(s * ncoltiles + ct) * RB + j]
+    // says that row RB i + j of that column holds data; unset = never written by the spreading kernel = zeros.
     const unsigned* row_masks;
     int ncoltiles;
     int set_of_trans_first;    // transforms [0, set_of_trans_first) belong to set 0 (x2), the rest to set 1 (x1)
@@ -149,56 +182,66 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
     }
 }
 
-// Pass 1, pruned and persistent: outer = 1, inner = n / 256.  Each CTA walks column tiles (16 columns x 256
-// rows of one transform); the 16-bit liveness mask of the NEXT tile is fetched while the current one is in
-// flight, so the mask never sits on the critical path.  Dead rows are not loaded (they were never written).
+// Pass 1, pruned and persistent: radix R1 = 16 RB over l1 (row stride inner = 65536 cells), C = 256 / RB
+// columns per tile, so a tile is always 4096 points = 256 threads x 16.  Stage 1: 16-point FFTs over i (rows
+// RB i + j); stage 2: RB-point FFTs over j.  The 16-bit liveness mask of the NEXT tile is fetched while the
+// current one is in flight, so it never sits on the critical path; dead rows are not loaded (never written).
+template <int RB>
 __global__ void __launch_bounds__(kFftThreads, 512 / kFftThreads)
 ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int ntiles_total) {
+    constexpr int C = 256 / RB, NI = 16 / RB, TWS = 16 / RB;   // TWS: stride of w_{R1} in the w_256 table
+    static_assert(kFftThreads == 256, "pass 1 is written for 256 threads");
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
-    double2* w256 = Y + 256 * kC;
+    double2* w256 = Y + 4096;
     fill_w256(w256);
-    const int c = threadIdx.x % kC, hi4 = threadIdx.x / kC;
+    const int c = threadIdx.x % C, hi = threadIdx.x / C;     // hi: j in stage 1, item group in stage 2
     auto mask_of = [&](int tile) -> unsigned {
         if (tile >= ntiles_total) return 0u;
         const int tr = tile / tiles_per_trans;
-        const long long m0 = (long long)(tile - tr * tiles_per_trans) * kC;
+        const long long m0 = (long long)(tile - tr * tiles_per_trans) * C;
         const int set = tr < a.set_of_trans_first ? 0 : 1;
-        return __ldg(&a.row_masks[((long long)set * a.ncoltiles + (m0 >> a.tile_shift)) * 16 + hi4]);
+        return __ldg(&a.row_masks[((long long)set * a.ncoltiles + (m0 >> a.tile_shift)) * RB + hi]);
     };
     int tile = blockIdx.x;
     unsigned live = mask_of(tile);
     __syncthreads();                                         // w256 ready
     for (; tile < ntiles_total; tile += gridDim.x) {
         const int tr = tile / tiles_per_trans;
-        const long long m = (long long)(tile - tr * tiles_per_trans) * kC + c;
+        const long long m = (long long)(tile - tr * tiles_per_trans) * C + c;
         double2* base = a.grids + (long long)tr * a.n + m;
-        double2 x[16];
         {
-            const int j = hi4;
+            const int j = hi;
+            double2 x[16];
 #pragma unroll
             for (int i = 0; i < 16; ++i) {
                 x[i] = make_double2(0.0, 0.0);
-                if (live >> i & 1u) x[i] = base[(long long)(16 * i + j) * inner];
+                if (live >> i & 1u) x[i] = base[(long long)(RB * i + j) * inner];
             }
             live = mask_of(tile + gridDim.x);                // prefetch: lands during this tile's work
             fft16(x);
 #pragma unroll
-            for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+            for (int ka = 0; ka < 16; ++ka)
+                Y[(ka * RB + j) * C + c] = cmul(x[pos16(ka)], w256[(j * ka * TWS) & 255]);
         }
         __syncthreads();
         {
-            const int ka = hi4;
-#pragma unroll
-            for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * kC + c];
-            fft16(x);
             const unsigned mm = (unsigned)m;
-            double2 tw = twiddle_n(a, (unsigned)ka * mm);
             const double2 st = twiddle_n(a, 16u * mm);
 #pragma unroll
-            for (int kb = 0; kb < 16; ++kb) {
-                base[(long long)(ka + 16 * kb) * inner] = cmul(x[pos16(kb)], tw);
-                tw = cmul(tw, st);
+            for (int q = 0; q < NI; ++q) {
+                const int ka = hi * NI + q;
+                double2 y[RB];
+#pragma unroll
+                for (int j = 0; j < RB; ++j) y[j] = Y[(ka * RB + j) * C + c];
+                fft_small<RB>(y);
+                // k1 = ka + 16 kb;  twiddle exponent k1 * m = ka m + kb (16 m)
+                double2 tw = twiddle_n(a, (unsigned)ka * mm);
+#pragma unroll
+                for (int kb = 0; kb < RB; ++kb) {
+                    base[(long long)(ka + 16 * kb) * inner] = cmul(y[fft_pos<RB>(kb)], tw);
+                    tw = cmul(tw, st);
+                }
             }
         }
         __syncthreads();                                     // Y is reused by the next tile
@@ -299,14 +342,24 @@ constexpr size_t kRowsSmem = sizeof(double2) * (256 * (kC + 1) + 256);
 
 }  // namespace
 
-bool own_fft_supported(const ls_plan_s* p) { return p->dtype == LS_F64 && p->n == ((int64_t)1 << 24); }
+// fp64 grids of 2^20 .. 2^24 cells: n = R1 * 256 * 256 with R1 = 16 .. 256 (pass 1 radix), spreading tiles that
+// divide a pass-1 row of 65536 cells.
+bool own_fft_supported(const ls_plan_s* p) {
+    const bool pow2 = (p->n & (p->n - 1)) == 0;
+    return p->dtype == LS_F64 && pow2 && p->n >= ((int64_t)1 << 20) && p->n <= ((int64_t)1 << 24) && 65536 % p->L == 0;
+}
+int own_fft_rb(const ls_plan_s* p) { return (int)(p->n >> 20); }
 
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     const int cnt = (int)std::max<long long>(4096, p->n / 4096);
     ls_fft_tables_kernel<<<(cnt + 255) / 256, 256, 0, s>>>((double2*)p->fft_wlo, (double2*)p->fft_whi, p->n);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(ls_fft_rows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem);
@@ -315,11 +368,12 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
 static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.grids = (double2*)p->grids + (long long)slot0 * p->n;
     a.n = p->n;
-    a.R1 = a.R2 = a.R3 = 256;
+    a.R1 = (int)(p->n >> 16);
+    a.R2 = a.R3 = 256;
     a.wlo = (const double2*)p->fft_wlo;
     a.whi = (const double2*)p->fft_whi;
     a.row_masks = p->row_masks;
-    a.ncoltiles = (int)(p->n / 256 / p->L);
+    a.ncoltiles = 65536 / p->L;
     a.set_of_trans_first = n_x2;
     a.tile_shift = 0;
     while ((1 << a.tile_shift) < p->L) ++a.tile_shift;
@@ -338,19 +392,25 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot0, n_x2);
-    const long long inner1 = p->n / 256;
-    const int tiles_per_trans = (int)(inner1 / kC), total = tiles_per_trans * ntrans;
-    ls_fft_pass1_kernel<<<std::min(total, (512 / kFftThreads) * p->num_sms), kFftThreads, kColsSmem, s>>>(
-        a, inner1, tiles_per_trans, total);
+    const long long inner1 = 65536;
+    const int rb = own_fft_rb(p);
+    const int tiles_per_trans = (int)(inner1 / (256 / rb)), total = tiles_per_trans * ntrans;
+    const int nblk = std::min(total, (512 / kFftThreads) * p->num_sms);
+    switch (rb) {
+        case 16: ls_fft_pass1_kernel<16><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 8: ls_fft_pass1_kernel<8><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 4: ls_fft_pass1_kernel<4><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 2: ls_fft_pass1_kernel<2><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
+        default: ls_fft_pass1_kernel<1><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
+    }
     return cudaGetLastError();
 }
 
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot0, 0);
-    const long long inner2 = p->n / 65536;
-    dim3 g2((unsigned)(inner2 / kC), 256, ntrans);
-    ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, 256, inner2);
+    dim3 g2(256 / kC, a.R1, ntrans);                       // [k1][l2][l3]: outer = R1 blocks, stride 256
+    ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, a.R1, 256);
     return cudaGetLastError();
 }
 
@@ -359,7 +419,7 @@ cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream
     if (ntrans <= 0) return cudaSuccess;
     FftArgs a;
     fill_common(p, a, slot0, 0);
-    dim3 g3(256 / kC, 256, ntrans);
+    dim3 g3(a.R1 / kC, 256, ntrans);
     ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
@@ -374,7 +434,7 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
     a.w2_modes = (const double2*)p->modes + (long long)w2_slot * p->Nf;
     a.power = (double*)power;
     a.series0 = series0;
-    dim3 g3(256 / kC, 256, nseries);
+    dim3 g3(a.R1 / kC, 256, nseries);
     ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }

@@ -108,12 +108,12 @@ struct ls_plan_s {
     size_t total_bytes = 0;
     size_t grids_bytes = 0, modes_bytes = 0;
     bool external_ws = false;   // grids / modes / fft_work live in caller memory (ls_set_workspace)
-    // own FFT (ls_fft.cu): n = 2^24 fp64; opts.fft_impl
+    // own FFT (ls_fft.cu): n = 2^20 .. 2^24, fp64; opts.fft_impl
     bool own_fft = false;
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
     void* modes = nullptr;                          // [slots][Nf] complex: kept modes in frequency order
-    unsigned* row_masks = nullptr;                  // [2][n/256/L][16] liveness bits for FFT pass 1 (in `zeroed`)
+    unsigned* row_masks = nullptr;                  // [2][65536/L][<=16] liveness bits for FFT pass 1 (in `zeroed`)
     // CUDA-graph replay of the execute sequence (launch-latency-bound small problems; opts.graph)
     bool use_graph = false;
     cudaGraphExec_t gexec = nullptr;
@@ -140,8 +140,9 @@ cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_
 cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int row0_x1, int nrows_x1,
                           int slot0_x1, cudaStream_t s);
 int spread_rows_per_group(const ls_plan_s* p);
-// ---- ls_fft.cu: own three-pass FFT (n = 2^24, fp64) ------------------------------------------
+// ---- ls_fft.cu: own three-pass FFT (n = 2^20 .. 2^24, fp64) ------------------------------------------
 bool own_fft_supported(const ls_plan_s* p);
+int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 = n / 2^20
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s);
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);

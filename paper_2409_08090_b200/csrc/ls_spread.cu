@@ -16,9 +16,10 @@
 //      kernel parameters; even/odd symmetry gives two values per evaluation) and stores them, with
 //      the NS complex strengths, at its slot;
 //   4. every thread then owns CPT consecutive cells, accumulates them in REGISTERS from the
-//      slot-ordered staging area and writes them once with 32-byte stores — zeros included.
-// There is no memset pass and no global or shared floating-point atomic; each grid cell is written
-// exactly once, and a tile without points is a pure streaming store.  One launch covers both point
+//      slot-ordered staging area and writes them once with 32-byte stores.
+// There is no memset pass and no global or shared floating-point atomic; each grid cell is written at
+// most once.  A tile without points is a pure streaming store of zeros when cuFFT follows; with the
+// library's own FFT it is not written at all (its liveness bit stays unset).  One launch covers both point
 // sets (blockIdx.y) and the tiles are visited in a permuted order so that compute-bound occupied
 // tiles and store-bound empty tiles overlap on every SM.
 #include "ls_internal.h"
@@ -59,7 +60,8 @@ struct SpreadArgs {
     int half;                        // ceil(w/2) stored polynomial pieces
     int skip_empty;                  // own FFT: tiles without points are flagged, not zero-filled
     unsigned* row_masks;             // own FFT: liveness bits of the written tiles (layout: ls_fft.cu FftArgs)
-    int ncoltiles, coltile_shift;    // tiles per FFT pass-1 row (n / 256 / L, a power of two) and its log2
+    int ncoltiles, coltile_shift;    // tiles per FFT pass-1 row (65536 / L) and its log2
+    int fft_rb;                      // pass-1 radix / 16: row = fft_rb * i + j
     long long Nd;
     SpreadSeg<T> seg[2];             // blockIdx.y < seg[0].ngroups: x2 rows, else x1 rows
     T c[kHalfMax][kMaxDeg + 1];      // only degrees <= PolyDeg<T> are read
@@ -245,7 +247,7 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
         if (total == 0) return;
         if (row0 == 0 && threadIdx.x == 0) {
             const int row = tile >> a.coltile_shift, ct = tile & (a.ncoltiles - 1);
-            atomicOr(&a.row_masks[(si * a.ncoltiles + ct) * 16 + (row & 15)], 1u << (row >> 4));
+            atomicOr(&a.row_masks[(si * a.ncoltiles + ct) * a.fft_rb + (row % a.fft_rb)], 1u << (row / a.fft_rb));
         }
     }
 
@@ -392,7 +394,8 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.half = p->poly.half;
     a.skip_empty = p->own_fft ? 1 : 0;
     a.row_masks = p->row_masks;
-    a.ncoltiles = (int)std::max<int64_t>(1, p->n / 256 / p->L);
+    a.ncoltiles = std::max(1, 65536 / p->L);
+    a.fft_rb = p->own_fft ? own_fft_rb(p) : 1;
     a.coltile_shift = 0;
     while ((1 << a.coltile_shift) < a.ncoltiles) ++a.coltile_shift;
     a.Nd = p->Nd;

@@ -102,6 +102,28 @@ def test_own_fft_batch_in_two_passes_at_headline_size():
     _check64(errors(Pb[2][ks], oracle_power(w2, ks=ks)))
 
 
+@pytest.mark.parametrize("p", [20, 21, 22, 23])
+def test_own_fft_other_power_of_two_grids(p):
+    """n = 2^p, p = 20..23: first-pass radix 16, 32, 64, 128 (ls_fft_pass1_kernel<RB>), against cuFFT on the
+    full grid and against the oracle on sampled frequencies."""
+    rng = np.random.default_rng(400 + p)
+    Nf = int(0.7 * (1 << p))
+    Nd = Nf // 12
+    t = rng.uniform(0, 2000.0, Nd)
+    dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    kg = Nf // 3
+    y = np.sin(2 * np.pi * (df + kg * df) * t + 0.4) + rng.normal(0, 1.0, Nd)
+    w = _custom(t, y, dy, df, df, Nf)
+    P_own, ex = gpu_power(w, fft_impl=2, no_autotune=1, return_plan_info=True)
+    assert ex["info"]["n"] == 1 << p and ex["launches"][1] == 0
+    P_cu = gpu_power(w, fft_impl=1, no_autotune=1)
+    assert np.max(np.abs(P_own - P_cu)) / P_cu.max() <= 1e-11
+    ks = np.unique(np.concatenate([compare_indices(w, 200), np.arange(kg - 3, kg + 4)]))
+    _check64(errors(P_own[0][ks], oracle_power(w, ks=ks)))
+    assert int(np.argmax(P_own[0])) == kg
+
+
 def test_own_fft_rejected_where_unsupported():
     from gpu_util import require_cuda
     require_cuda()
