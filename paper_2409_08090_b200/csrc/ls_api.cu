@@ -301,6 +301,7 @@ int ls_destroy(ls_plan_t p) {
     cudaFree(p->dinv);
     cudaFree(p->fft_wlo);
     cudaFree(p->fft_whi);
+    cudaFree(p->tile_list);
     cudaFree(p->zeroed);                     // sums and both histograms live in this allocation
     cudaFree(p->scan_tmp);
     for (int i = 0; i < 2; ++i) {
@@ -441,10 +442,14 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
-        const size_t mask_bytes = p->own_fft ? (size_t)2 * (65536 / p->L) * 16 * 4 : 0;
+        const size_t mask_bytes = p->own_fft ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : 0;   // masks + 2 list counters
         p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
-        if (p->own_fft) p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes);
+        if (p->own_fft) {
+            p->tile_counts = (int*)((char*)p->zeroed + sums_bytes + hist_bytes);
+            p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes + 256);
+            if ((ce = dmalloc(p, &p->tile_list, (size_t)2 * p->ntiles * 4)) != cudaSuccess) break;
+        }
         p->sums = (double*)p->zeroed;
         p->ps[0].hist = (int*)((char*)p->zeroed + sums_bytes);
         p->ps[1].hist = p->ps[0].hist + p->nbins;
@@ -537,6 +542,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
 
     stage_begin(p, LS_STAGE_SORT, s);
     LS_TRY(lsb::launch_bin_scan(p, s)); own += 2;
+    if (p->own_fft) { LS_TRY(lsb::launch_tile_list(p, s)); ++own; }
     stage_end(p, s);
 
     stage_begin(p, LS_STAGE_PREMUL, s);

@@ -113,6 +113,8 @@ struct ls_plan_s {
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
     void* modes = nullptr;                          // [slots][Nf] complex: kept modes in frequency order
+    int* tile_list = nullptr;                       // [2][ntiles] occupied spreading tiles per point set (x2, x1)
+    int* tile_counts = nullptr;                     // [2] list lengths (in `zeroed`)
     unsigned* row_masks = nullptr;                  // [2][65536/L][<=16] liveness bits for FFT pass 1 (in `zeroed`)
     // CUDA-graph replay of the execute sequence (launch-latency-bound small problems; opts.graph)
     bool use_graph = false;
@@ -140,6 +142,7 @@ cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_
 cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int row0_x1, int nrows_x1,
                           int slot0_x1, cudaStream_t s);
 int spread_rows_per_group(const ls_plan_s* p);
+cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s);
 // ---- ls_fft.cu: own three-pass FFT (n = 2^20 .. 2^24, fp64) ------------------------------------------
 bool own_fft_supported(const ls_plan_s* p);
 int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 = n / 2^20

@@ -62,6 +62,8 @@ struct SpreadArgs {
     unsigned* row_masks;             // own FFT: liveness bits of the written tiles (layout: ls_fft.cu FftArgs)
     int ncoltiles, coltile_shift;    // tiles per FFT pass-1 row (65536 / L) and its log2
     int fft_rb;                      // pass-1 radix / 16: row = fft_rb * i + j
+    const int* tile_list;            // own FFT: [2][ntiles] tiles that hold points, per point set (x2, x1)
+    const int* tile_counts;          // own FFT: [2] lengths of the two lists
     long long Nd;
     SpreadSeg<T> seg[2];             // blockIdx.y < seg[0].ngroups: x2 rows, else x1 rows
     T c[kHalfMax][kMaxDeg + 1];      // only degrees <= PolyDeg<T> are read
@@ -194,6 +196,47 @@ __device__ __forceinline__ void gather_cells(typename V2<T>::type (&acc)[NS][CPT
     }
 }
 
+// Candidates of the tile [tile_lo, tile_lo + Lt): the points of the sort bins overlapping cells
+// [lo, hi) = [tile_lo - H, tile_lo + Lt + H).  Main piece = the part inside [0, n); the parts below 0 / at
+// or above n are periodic images (pieces 1 and 2, cell shift -n / +n).  Returns the total count.
+__device__ __forceinline__ int tile_candidates(const int* __restrict__ bin_start, int n, int nbins, int H, int tile_lo,
+                                               int Lt, int& pbeg0, int& pcnt0, int& pbeg1, int& pcnt1, int& pcnt2) {
+    const int lo = tile_lo - H, hi = tile_lo + Lt + H;
+    pbeg1 = 0; pcnt1 = 0; pcnt2 = 0;
+    if (lo >= 0 && hi <= n) {                        // interior tile: two loads, no images
+        pbeg0 = __ldg(&bin_start[(unsigned)lo / kBinCells]);
+        pcnt0 = __ldg(&bin_start[(unsigned)(hi - 1) / kBinCells + 1]) - pbeg0;
+    } else {
+        const int mlo = max(lo, 0), mhi = min(hi, n);
+        pbeg0 = __ldg(&bin_start[mlo / kBinCells]);
+        pcnt0 = __ldg(&bin_start[(mhi - 1) / kBinCells + 1]) - pbeg0;
+        if (lo < 0) {                                // left image: cells [n + lo, n) shifted by -n
+            pbeg1 = __ldg(&bin_start[max(n + lo, 0) / kBinCells]);
+            pcnt1 = __ldg(&bin_start[nbins]) - pbeg1;
+        }
+        if (hi > n)                                  // right image: cells [0, hi - n) shifted by +n
+            pcnt2 = __ldg(&bin_start[(min(hi - n, n) - 1) / kBinCells + 1]);
+    }
+    return pcnt0 + pcnt1 + pcnt2;
+}
+
+// Own-FFT path: the tiles that hold points, listed per point set (so that the spreading kernel launches
+// work for them only), and their liveness bits for the first FFT pass.  One thread per (set, tile).
+__global__ void ls_tile_list_kernel(const int* __restrict__ bin_start_x2, const int* __restrict__ bin_start_x1, int n,
+                                    int nbins, int H, int L, int ntiles, int* __restrict__ list, int* __restrict__ counts,
+                                    unsigned* __restrict__ row_masks, int ncoltiles, int coltile_shift, int fft_rb) {
+    const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= 2 * ntiles) return;
+    const int set = idx >= ntiles ? 1 : 0, tile = idx - set * ntiles;
+    const int tile_lo = tile * L;
+    int b0, c0, b1, c1, c2;
+    if (tile_candidates(set ? bin_start_x1 : bin_start_x2, n, nbins, H, tile_lo, min(L, n - tile_lo), b0, c0, b1, c1, c2) == 0)
+        return;
+    list[set * ntiles + atomicAdd(&counts[set], 1)] = tile;
+    const int row = tile >> coltile_shift, ct = tile & (ncoltiles - 1);
+    atomicOr(&row_masks[(set * ncoltiles + ct) * fft_rb + (row % fft_rb)], 1u << (row / fft_rb));
+}
+
 template <typename T, int NS, int CPT>
 __global__ void __launch_bounds__(kSpreadThreads, (NS * CPT <= 8) ? 4 : 3)
 ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
@@ -211,53 +254,44 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     int* start = cnt + HN;
     int* warp_tot = start + HN + 1;
 
-    // Occupied tiles (compute/latency-bound) and empty tiles (pure streaming stores) are interleaved in
-    // launch order by a multiplicative permutation, so the two kinds of work overlap on every SM.
-    int tile;
-    if (a.tile_mask >= 0) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) & (unsigned)a.tile_mask);
-    else if (a.ntiles <= 65535) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) % (unsigned)a.ntiles);
-    else tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
-    const int si = (int)blockIdx.y < a.seg[0].ngroups ? 0 : 1;
+    // Work items.  cuFFT path: one CTA per (tile, row group), tiles visited in a permuted order so that occupied
+    // tiles (compute/latency-bound) and empty tiles (pure streaming stores of zeros) interleave on every SM.
+    // Own-FFT path: empty tiles do not exist; a persistent grid walks the (listed tile, row group) pairs.
+    int n2 = 0, nitems = 1;
+    if (a.skip_empty) {
+        n2 = __ldg(&a.tile_counts[0]) * a.seg[0].ngroups;
+        nitems = n2 + __ldg(&a.tile_counts[1]) * a.seg[1].ngroups;
+    }
+    const int lbase = threadIdx.x * CPT;             // first owned cell, tile-relative
+    for (int item = blockIdx.x; item < nitems || !a.skip_empty; item += gridDim.x) {
+    int tile, si, grp;
+    if (a.skip_empty) {
+        si = item < n2 ? 0 : 1;
+        const int e = si ? item - n2 : item, ng = a.seg[si].ngroups;
+        grp = e % ng;
+        tile = __ldg(&a.tile_list[si * a.ntiles + e / ng]);
+    } else {
+        if (item != (int)blockIdx.x) break;          // one item per CTA
+        if (a.tile_mask >= 0) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) & (unsigned)a.tile_mask);
+        else if (a.ntiles <= 65535) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) % (unsigned)a.ntiles);
+        else tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
+        si = (int)blockIdx.y < a.seg[0].ngroups ? 0 : 1;
+        grp = (int)blockIdx.y - (si ? a.seg[0].ngroups : 0);
+    }
     const SpreadSeg<T>& sg = a.seg[si];
-    const int row0 = ((int)blockIdx.y - (si ? a.seg[0].ngroups : 0)) * NS;
+    const int row0 = grp * NS;
     const int nr = min(NS, sg.nrows - row0);
     const int tile_lo = tile * a.L;
     const int Lt = min(a.L, a.n - tile_lo);
 
-    // Candidate pieces: cells [lo, hi) = [tile_lo - H, tile_lo + Lt + H); the parts below 0 / at or
-    // above n are the periodic images (shift -n / +n applied to the point's cell).
-    const int lo = tile_lo - a.H, hi = tile_lo + Lt + a.H;
-    int pbeg0, pcnt0, pbeg1 = 0, pcnt1 = 0, pcnt2 = 0;
-    if (lo >= 0 && hi <= a.n) {                      // interior tile: two loads, no images
-        pbeg0 = __ldg(&sg.bin_start[(unsigned)lo / kBinCells]);
-        pcnt0 = __ldg(&sg.bin_start[(unsigned)(hi - 1) / kBinCells + 1]) - pbeg0;
-    } else {
-        const int mlo = max(lo, 0), mhi = min(hi, a.n);
-        pbeg0 = __ldg(&sg.bin_start[mlo / kBinCells]);
-        pcnt0 = __ldg(&sg.bin_start[(mhi - 1) / kBinCells + 1]) - pbeg0;
-        if (lo < 0) {                                // left image: cells [n + lo, n) shifted by -n
-            pbeg1 = __ldg(&sg.bin_start[max(a.n + lo, 0) / kBinCells]);
-            pcnt1 = __ldg(&sg.bin_start[a.nbins]) - pbeg1;
-        }
-        if (hi > a.n)                                // right image: cells [0, hi - n) shifted by +n
-            pcnt2 = __ldg(&sg.bin_start[(min(hi - a.n, a.n) - 1) / kBinCells + 1]);
-    }
-    const int total = pcnt0 + pcnt1 + pcnt2;
-    if (a.skip_empty) {                              // the own FFT's first pass never loads unflagged tiles
-        if (total == 0) return;
-        if (row0 == 0 && threadIdx.x == 0) {
-            const int row = tile >> a.coltile_shift, ct = tile & (a.ncoltiles - 1);
-            atomicOr(&a.row_masks[(si * a.ncoltiles + ct) * a.fft_rb + (row % a.fft_rb)], 1u << (row / a.fft_rb));
-        }
-    }
+    int pbeg0, pcnt0, pbeg1, pcnt1, pcnt2;
+    const int total = tile_candidates(sg.bin_start, a.n, a.nbins, a.H, tile_lo, Lt, pbeg0, pcnt0, pbeg1, pcnt1, pcnt2);
 
     T2 acc[NS][CPT];
 #pragma unroll
     for (int s = 0; s < NS; ++s)
 #pragma unroll
         for (int c = 0; c < CPT; ++c) acc[s][c].x = acc[s][c].y = (T)0;
-
-    const int lbase = threadIdx.x * CPT;             // first owned cell, tile-relative
 
     for (int base = 0; base < total; base += kChunkPts) {
         // ---- 1. one candidate per thread: its record and strengths (loads issued before the barrier)
@@ -336,7 +370,7 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
         if (base + kChunkPts < total) __syncthreads();   // staging area is reused by the next chunk
     }
 
-    // ---- 5. the tile is written exactly once (zeros included)
+    // ---- 5. the tile is written exactly once
     if (lbase < Lt) {
 #pragma unroll
         for (int s = 0; s < NS; ++s) {
@@ -352,6 +386,7 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
             }
         }
     }
+    }   // work items (the next item's first barrier orders its shared-memory writes after this item's reads)
 }
 
 template <typename T, int NS>
@@ -372,6 +407,10 @@ cudaError_t launch_inst(ls_plan_s* p, const SpreadArgs<T>& a, cudaStream_t s) {
         configured[dev] = true;
     }
     dim3 grid(p->ntiles, a.seg[0].ngroups + a.seg[1].ngroups);
+    if (a.skip_empty) {                              // persistent: as many CTAs as fit, never more than the work
+        const long long items = (long long)p->ntiles * (a.seg[0].ngroups + a.seg[1].ngroups);
+        grid = dim3((unsigned)std::min<long long>(items, (long long)p->num_sms * ((NS * CPT <= 8) ? 4 : 3)));
+    }
     ls_spread_tile_kernel<T, NS, CPT><<<grid, kSpreadThreads, spread_smem_bytes<T, NS>(p->L, p->w), s>>>(a);
     return cudaGetLastError();
 }
@@ -394,6 +433,8 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.half = p->poly.half;
     a.skip_empty = p->own_fft ? 1 : 0;
     a.row_masks = p->row_masks;
+    a.tile_list = p->tile_list;
+    a.tile_counts = p->tile_counts;
     a.ncoltiles = std::max(1, 65536 / p->L);
     a.fft_rb = p->own_fft ? own_fft_rb(p) : 1;
     a.coltile_shift = 0;
@@ -422,6 +463,18 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
 }
 
 }  // namespace
+
+// Own-FFT path, once per execute after the bin scan: occupied-tile lists and liveness masks of both point sets.
+cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s) {
+    const int ncol = std::max(1, 65536 / p->L);
+    int shift = 0;
+    while ((1 << shift) < ncol) ++shift;
+    const int total = 2 * p->ntiles;
+    ls_tile_list_kernel<<<(total + 255) / 256, 256, 0, s>>>(p->ps[1].bin_start, p->ps[0].bin_start, (int)p->n, p->nbins,
+                                                           (p->w + 1) / 2, p->L, p->ntiles, p->tile_list, p->tile_counts,
+                                                           p->row_masks, ncol, shift, own_fft_rb(p));
+    return cudaGetLastError();
+}
 
 // Transforms accumulated per CTA: 2 for a single series ({w, h} at x1), 4 for a batch.
 int spread_rows_per_group(const ls_plan_s* p) { return p->batch == 1 ? 2 : 4; }
