@@ -257,19 +257,51 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
     // Work items.  cuFFT path: one CTA per (tile, row group), tiles visited in a permuted order so that occupied
     // tiles (compute/latency-bound) and empty tiles (pure streaming stores of zeros) interleave on every SM.
     // Own-FFT path: empty tiles do not exist; a persistent grid walks the (listed tile, row group) pairs.
-    int n2 = 0, nitems = 1;
+    // Persistent order: the x1 items first (two transforms and, at the same point density, twice the
+    // candidates per tile: longest first shortens the tail), then the x2 items.
+    int n1 = 0, nitems = 1;
     if (a.skip_empty) {
-        n2 = __ldg(&a.tile_counts[0]) * a.seg[0].ngroups;
-        nitems = n2 + __ldg(&a.tile_counts[1]) * a.seg[1].ngroups;
+        n1 = __ldg(&a.tile_counts[1]) * a.seg[1].ngroups;
+        nitems = n1 + __ldg(&a.tile_counts[0]) * a.seg[0].ngroups;
     }
     const int lbase = threadIdx.x * CPT;             // first owned cell, tile-relative
+    // Two-deep prefetch down the item list: the tile id of item i + 2G and the candidate ranges of item
+    // i + G are requested while item i is processed, so neither dependent load sits on the critical path.
+    auto item_tile = [&](int it) -> int {
+        if (it >= nitems) return 0;
+        const int s_ = it < n1 ? 1 : 0, e = s_ ? it : it - n1;
+        return __ldg(&a.tile_list[s_ * a.ntiles + e / a.seg[s_].ngroups]);
+    };
+    struct Cand { int pbeg0, pcnt0, pbeg1, pcnt1, pcnt2, total; };
+    auto item_cand = [&](int it, int tl) -> Cand {
+        Cand c{0, 0, 0, 0, 0, 0};
+        if (it < nitems) {
+            const int tlo = tl * a.L;
+            c.total = tile_candidates(a.seg[it < n1 ? 1 : 0].bin_start, a.n, a.nbins, a.H, tlo, min(a.L, a.n - tlo),
+                                      c.pbeg0, c.pcnt0, c.pbeg1, c.pcnt1, c.pcnt2);
+        }
+        return c;
+    };
+    int tile_cur = 0, tile_nx = 0;
+    Cand cand_cur{0, 0, 0, 0, 0, 0};
+    if (a.skip_empty) {
+        tile_cur = item_tile(blockIdx.x);
+        tile_nx = item_tile(blockIdx.x + gridDim.x);
+        cand_cur = item_cand(blockIdx.x, tile_cur);
+    }
     for (int item = blockIdx.x; item < nitems || !a.skip_empty; item += gridDim.x) {
     int tile, si, grp;
+    int pbeg0, pcnt0, pbeg1, pcnt1, pcnt2, total;
+    int tile_nx2 = 0;
+    Cand cand_nx{0, 0, 0, 0, 0, 0};
     if (a.skip_empty) {
-        si = item < n2 ? 0 : 1;
-        const int e = si ? item - n2 : item, ng = a.seg[si].ngroups;
-        grp = e % ng;
-        tile = __ldg(&a.tile_list[si * a.ntiles + e / ng]);
+        si = item < n1 ? 1 : 0;
+        grp = (si ? item : item - n1) % a.seg[si].ngroups;
+        tile = tile_cur;
+        pbeg0 = cand_cur.pbeg0; pcnt0 = cand_cur.pcnt0; pbeg1 = cand_cur.pbeg1; pcnt1 = cand_cur.pcnt1;
+        pcnt2 = cand_cur.pcnt2; total = cand_cur.total;
+        tile_nx2 = item_tile(item + 2 * gridDim.x);
+        cand_nx = item_cand(item + gridDim.x, tile_nx);
     } else {
         if (item != (int)blockIdx.x) break;          // one item per CTA
         if (a.tile_mask >= 0) tile = (int)((blockIdx.x * (unsigned)a.tile_stride) & (unsigned)a.tile_mask);
@@ -277,15 +309,15 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
         else tile = (int)(((long long)blockIdx.x * a.tile_stride) % a.ntiles);
         si = (int)blockIdx.y < a.seg[0].ngroups ? 0 : 1;
         grp = (int)blockIdx.y - (si ? a.seg[0].ngroups : 0);
+        const int tlo = tile * a.L;
+        total = tile_candidates(a.seg[si].bin_start, a.n, a.nbins, a.H, tlo, min(a.L, a.n - tlo), pbeg0, pcnt0, pbeg1,
+                                pcnt1, pcnt2);
     }
     const SpreadSeg<T>& sg = a.seg[si];
     const int row0 = grp * NS;
     const int nr = min(NS, sg.nrows - row0);
     const int tile_lo = tile * a.L;
     const int Lt = min(a.L, a.n - tile_lo);
-
-    int pbeg0, pcnt0, pbeg1, pcnt1, pcnt2;
-    const int total = tile_candidates(sg.bin_start, a.n, a.nbins, a.H, tile_lo, Lt, pbeg0, pcnt0, pbeg1, pcnt1, pcnt2);
 
     T2 acc[NS][CPT];
 #pragma unroll
@@ -386,6 +418,9 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
             }
         }
     }
+    tile_cur = tile_nx;
+    tile_nx = tile_nx2;
+    cand_cur = cand_nx;
     }   // work items (the next item's first barrier orders its shared-memory writes after this item's reads)
 }
 
