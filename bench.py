@@ -56,6 +56,7 @@ def parse_args():
     ap.add_argument("--kernel-width", type=int, default=0)
     ap.add_argument("--batch-chunk", type=int, default=0)
     ap.add_argument("--fft-impl", type=int, default=0, help="0 auto, 1 cuFFT, 2 own three-pass FFT")
+    ap.add_argument("--graph", type=int, default=0, help="0 auto, 1 never, 2 always (user-facing plan)")
     return ap.parse_args()
 
 
@@ -297,7 +298,7 @@ def run_ours(args):
     # the last pass is fused with the assembly) and gives `value`; `plan_t` records CUDA events around every
     # stage and gives stage_ms / the roofline legs — same n, w and FFT, but with the assembly as its own kernel
     # (fft_impl 3) so that "fft" and "assemble" are cleanly separated as north_star asks.
-    plan = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, ldt, w.batch, timing=0, **popts)
+    plan = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, ldt, w.batch, timing=0, graph=args.graph, **popts)
     info = plan.info
     if not args.upsampfac:
         popts["upsampfac"] = info["n"] / w.Nf * (1 - 1e-12) if info["n"] & (info["n"] - 1) else 0.0   # same n as `plan`

@@ -86,8 +86,9 @@ typedef struct {
     int tile_cells;         /* spreading tile length L in cells; 0 = auto                         */
     int batch_chunk;        /* series spread/FFT'd/assembled per pass; 0 = auto (<= 8 GB of grids)  */
     int no_autotune;        /* 1: never time candidate grid sizes at plan time (auto n = power of two) */
-    int graph;              /* 0 = auto: small problems replay a captured CUDA graph when timing == 0;
-                               1 = never, 2 = always (when timing == 0)                            */
+    int graph;              /* CUDA-graph replay of the execute sequence (needs timing == 0 and a non-legacy
+                               stream): 0 = auto (on; off for good after three consecutive executes
+                               with changed buffer pointers), 1 = never, 2 = always                 */
     int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs an
                                fp64 grid of 2^20..2^24 cells; LS_ERR_UNSUPPORTED otherwise), 3 = as 2 but with
                                deconvolution + assembly as a separate kernel (clean stage timings)  */

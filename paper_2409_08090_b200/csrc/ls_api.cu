@@ -424,7 +424,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     p->model_bytes = 8.0 * Nd + (double)batch * Nd * B + (per ? (double)batch : 1.0) * Nd * B + 8.0 * Nd +
                      (double)p->M * p->n * 2 * B + (double)p->M * Nf * 2 * B + (double)batch * Nf * B;
 
-    p->use_graph = !o.timing && (o.graph == 2 || (o.graph == 0 && p->model_bytes < 256e6));
+    p->use_graph = !o.timing && o.graph != 1;
 
     int rc = LS_OK;
     cudaError_t ce = cudaSuccess;
@@ -624,6 +624,13 @@ int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* 
     // A legacy default stream cannot be captured; any capture failure falls back to direct launches for good.
     if (!p->use_graph || s == nullptr) return enqueue_execute(p, t, y, dy, power, s);
     if (!p->gexec || p->g_t != t || p->g_y != y || p->g_dy != dy || p->g_power != power) {
+        // auto mode: a caller that changes buffers on every call gains nothing from replay — stop capturing
+        if (p->gexec && p->opts.graph == 0 && ++p->g_misses >= 3) {
+            cudaGraphExecDestroy(p->gexec);
+            p->gexec = nullptr;
+            p->use_graph = false;
+            return enqueue_execute(p, t, y, dy, power, s);
+        }
         if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }
         cudaGraph_t graph = nullptr;
         int rc = LS_ERR_CUDA;
@@ -641,6 +648,7 @@ int ls_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* 
         }
         p->g_t = t; p->g_y = y; p->g_dy = dy; p->g_power = power;
     }
+    else p->g_misses = 0;
     if (cudaGraphLaunch(p->gexec, s) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
     return LS_OK;
 }

@@ -121,6 +121,7 @@ struct ls_plan_s {
     cudaGraphExec_t gexec = nullptr;
     const void *g_t = nullptr, *g_y = nullptr, *g_dy = nullptr;
     void* g_power = nullptr;
+    int g_misses = 0;           // consecutive executes that had to re-capture (auto mode gives up at 3)
     // timing
     std::vector<lsb::StageEvent> events;
     size_t events_used = 0;
