@@ -263,11 +263,20 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
     const double invW = 1.0 / W;
     for (long long j = (long long)blockIdx.x * kPreThreads + threadIdx.x; j < Nd;
          j += (long long)gridDim.x * kPreThreads) {
+        // all three loads first, the two slot atomics as soon as the cells are known: their latencies
+        // overlap each other and the phase arithmetic instead of lining up behind it
         const double tj = t[j];
+        double yj = 0.0, dj = 1.0;
+        if (FUSE_ROWS) {
+            yj = (double)y[j];
+            dj = (double)dy[j];
+        }
         int c1, c2, i1, i2;
         double f1, f2, xa, xb;
         grid_coord(ndf, tj, dn, c1, f1);
         grid_coord_x2(c1, f1, n, c2, f2);
+        const int s1 = atomicAdd(&cur1[c1 / kBinCells], 1);
+        const int s2 = atomicAdd(&cur2[c2 / kBinCells], 1);
         support_start(f1, w, i1, xa);
         support_start(f2, w, i2, xb);
         // phase of f_c t in cycles, reduced to [-0.5, 0.5] (double-double product)
@@ -277,15 +286,12 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
         ph -= rint(ph);
         double sn, cs;
         sincospi(2.0 * ph, &sn, &cs);
-        const int s1 = atomicAdd(&cur1[c1 / kBinCells], 1);
-        const int s2 = atomicAdd(&cur2[c2 / kBinCells], 1);
         // eta = 2 (x0 + w/2) - 1 in [-1, 1): argument of the piecewise-polynomial kernel
         store_rec(&rec1[s1], 2.0 * xa + (double)(w - 1), c1 + i1, cs, sn);
         store_rec(&rec2[s2], 2.0 * xb + (double)(w - 1), c2 + i2, cs * cs - sn * sn, 2.0 * sn * cs);
         if (FUSE_ROWS) {
-            const double d = (double)dy[j];
-            const double wj = invW / (d * d);
-            const double yc = (double)y[j] - ybar;
+            const double wj = invW / (dj * dj);
+            const double yc = yj - ybar;
             R1[s1] = (T)wj;                     // row 0 of x1: w
             R1[Nd + s1] = (T)(wj * yc);         // row 1 of x1: h
             R2[s2] = (T)wj;                     // row 0 of x2: w

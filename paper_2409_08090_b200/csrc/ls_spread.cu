@@ -232,9 +232,15 @@ __global__ void ls_tile_list_kernel(const int* __restrict__ bin_start_x2, const 
     int b0, c0, b1, c1, c2;
     if (tile_candidates(set ? bin_start_x1 : bin_start_x2, n, nbins, H, tile_lo, min(L, n - tile_lo), b0, c0, b1, c1, c2) == 0)
         return;
-    list[set * ntiles + atomicAdd(&counts[set], 1)] = tile;
     const int row = tile >> coltile_shift, ct = tile & (ncoltiles - 1);
     atomicOr(&row_masks[(set * ncoltiles + ct) * fft_rb + (row % fft_rb)], 1u << (row / fft_rb));
+    // one counter atomic per warp and set, not per tile (thousands of same-address atomics serialise)
+    const unsigned peers = __match_any_sync(__activemask(), set);
+    const int leader = __ffs(peers) - 1, lane = threadIdx.x & 31;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(&counts[set], __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    list[set * ntiles + base + __popc(peers & ((1u << lane) - 1))] = tile;
 }
 
 template <typename T, int NS, int CPT>
