@@ -458,9 +458,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         if ((ce = cudaMemset(p->scan_tmp, 0, (size_t)2 * (nchunks + 1) * 4)) != cudaSuccess) break;
         for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
             lsb::PointSet& ps = p->ps[i];
-            ps.nrows = i == 0 ? (per ? 2 * batch : batch + 1) : (per ? batch : 1);
+            // stored strength rows (shared dy: the weights live in the records, only y - ybar is stored)
+            ps.nrows = i == 0 ? (per ? 2 * batch : batch) : (per ? batch : 0);
             if ((ce = dmalloc(p, &ps.bin_start, (size_t)(p->nbins + 1) * 4)) != cudaSuccess) break;
-            if (batch > 1 && (ce = dmalloc(p, &ps.perm, (size_t)Nd * 4)) != cudaSuccess) break;
+            if ((batch > 1 || per) && (ce = dmalloc(p, &ps.perm, (size_t)Nd * 4)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&ps.rec, (size_t)Nd * 4 * B)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&ps.rows, (size_t)ps.nrows * Nd * B)) != cudaSuccess) break;
         }
@@ -547,7 +548,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
 
     stage_begin(p, LS_STAGE_PREMUL, s);
     LS_TRY(lsb::launch_premultiply(p, (const double*)t, y, dy, s)); ++own;
-    if (p->batch > 1) { LS_TRY(lsb::launch_rows(p, y, dy, s)); ++own; }
+    if (p->batch > 1 || per) { LS_TRY(lsb::launch_rows(p, y, dy, s)); ++own; }
     stage_end(p, s);
 
     {

@@ -57,9 +57,9 @@ struct __align__(16) Rec32 {
 struct PointSet {
     int* hist = nullptr;       // [nbins]   bin counts -> running cursors during the scatter
     int* bin_start = nullptr;  // [nbins+1] exclusive scan of the counts
-    int* perm = nullptr;       // [Nd]      input index of sorted slot s (batch > 1 only)
+    int* perm = nullptr;       // [Nd]      input index of sorted slot s (when a rows kernel runs)
     void* rec = nullptr;       // [Nd]      Rec64 / Rec32, sorted order
-    void* rows = nullptr;      // [nrows][Nd] T  real strengths per transform, sorted order
+    void* rows = nullptr;      // [nrows][Nd] T  stored real strengths, sorted order (shared dy: y - ybar only)
     int nrows = 0;
 };
 

@@ -243,10 +243,14 @@ __device__ __forceinline__ void store_rec(Rec32* dst, double eta, int l0, double
     *reinterpret_cast<float4*>(dst) = v;
 }
 
-// grid-stride over the points.  FUSE_ROWS (batch == 1): the strengths w_j, h_j = w_j (y_j - ybar) of
-// the single series are scattered here too and YY is reduced, so no separate rows kernel runs.
-// Otherwise the sorted slot -> input index map `perm` is written for the gathering rows kernel.
-template <typename T, bool FUSE_ROWS>
+// grid-stride over the points.
+// FOLD_W (dy shared by the batch): the record's phasor is w_j e^{2 pi i f_c t_j}, not the unit phasor, so
+//   the w transforms need no strength row at all (strength 1) and an h transform's strength is just
+//   y_j - ybar: one scattered 8-byte store per point instead of three (they were half of this kernel's time).
+// FUSE_ROWS (batch == 1): that one strength row of the single series is scattered here too and YY is
+//   reduced, so no separate rows kernel runs.  Otherwise the sorted slot -> input index map `perm` is
+//   written for the gathering rows kernel.
+template <typename T, bool FUSE_ROWS, bool FOLD_W>
 __global__ void __launch_bounds__(kPreThreads)
 ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, const T* __restrict__ dy,
                       double* __restrict__ sums, long long Nd, dd ndf, dd fc, int n, int w,
@@ -256,7 +260,7 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
     __shared__ double red[kPreThreads / 32];
     const double dn = (double)n;
     double W = 1.0, ybar = 0.0, yy = 0.0;
-    if (FUSE_ROWS) {
+    if (FUSE_ROWS || FOLD_W) {
         W = sums[0];
         ybar = sums[1] / W;
     }
@@ -267,10 +271,8 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
         // overlap each other and the phase arithmetic instead of lining up behind it
         const double tj = t[j];
         double yj = 0.0, dj = 1.0;
-        if (FUSE_ROWS) {
-            yj = (double)y[j];
-            dj = (double)dy[j];
-        }
+        if (FUSE_ROWS) yj = (double)y[j];
+        if (FOLD_W) dj = (double)dy[j];
         int c1, c2, i1, i2;
         double f1, f2, xa, xb;
         grid_coord(ndf, tj, dn, c1, f1);
@@ -286,19 +288,17 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
         ph -= rint(ph);
         double sn, cs;
         sincospi(2.0 * ph, &sn, &cs);
+        const double wj = FOLD_W ? invW / (dj * dj) : 1.0;
         // eta = 2 (x0 + w/2) - 1 in [-1, 1): argument of the piecewise-polynomial kernel
-        store_rec(&rec1[s1], 2.0 * xa + (double)(w - 1), c1 + i1, cs, sn);
-        store_rec(&rec2[s2], 2.0 * xb + (double)(w - 1), c2 + i2, cs * cs - sn * sn, 2.0 * sn * cs);
+        store_rec(&rec1[s1], 2.0 * xa + (double)(w - 1), c1 + i1, wj * cs, wj * sn);
+        store_rec(&rec2[s2], 2.0 * xb + (double)(w - 1), c2 + i2, wj * (cs * cs - sn * sn), wj * (2.0 * sn * cs));
         if (FUSE_ROWS) {
-            const double wj = invW / (dj * dj);
             const double yc = yj - ybar;
-            R1[s1] = (T)wj;                     // row 0 of x1: w
-            R1[Nd + s1] = (T)(wj * yc);         // row 1 of x1: h
-            R2[s2] = (T)wj;                     // row 0 of x2: w
+            R1[s1] = (T)yc;                     // the only stored row of x1: h / w = y - ybar
             yy += wj * yc * yc;
         } else {
             perm1[s1] = (int)j;
-            perm2[s2] = (int)j;
+            if (!FOLD_W) perm2[s2] = (int)j;
         }
     }
     if (FUSE_ROWS) {
@@ -309,9 +309,7 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
 
 // ------------------------------------------------------------------------------ K2' rows + YY
 // batch > 1.  grid (slot CTAs, batch), grid-stride over SORTED slots: coalesced row writes, gathers
-// of y and dy through perm (one series is Nd reals: L1/L2-resident).  Row layout:
-//   shared dy:      R1 = [w ; h_0 .. h_{B-1}],  R2 = [w]
-//   per-series dy:  R1 = [w_0, h_0, w_1, h_1, ...],  R2 = [w_0, w_1, ...]
+// of y and dy through perm (one series is Nd reals: L1/L2-resident).  Row layout: DESIGN.md §4.
 template <typename T>
 __global__ void __launch_bounds__(kPreThreads)
 ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __restrict__ sums,
@@ -324,10 +322,11 @@ ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __rest
     const double W = sums[dy_per_series ? 4 * s : 0];
     const double ybar = sums[4 * s + 1] / W;
     const double invW = 1.0 / W;
-    T* rowh = R1 + (long long)(dy_per_series ? 2 * s + 1 : 1 + s) * Nd;
-    T* roww1 = R1 + (long long)(dy_per_series ? 2 * s : 0) * Nd;
-    T* roww2 = R2 + (long long)(dy_per_series ? s : 0) * Nd;
-    const bool write_w = dy_per_series || s == 0;
+    // per-series dy: R1 = [w_0, h_0, w_1, h_1, ...], R2 = [w_0, w_1, ...], h_s = w_s (y_s - ybar_s);
+    // shared dy (weights folded into the records' phasors): R1 = [y_0 - ybar_0, y_1 - ybar_1, ...], no R2
+    T* rowh = R1 + (long long)(dy_per_series ? 2 * s + 1 : s) * Nd;
+    T* roww1 = R1 + (long long)(2 * s) * Nd;
+    T* roww2 = R2 + (long long)s * Nd;
     double yy = 0.0;
     for (long long q = (long long)blockIdx.x * kPreThreads + threadIdx.x; q < Nd;
          q += (long long)gridDim.x * kPreThreads) {
@@ -335,12 +334,14 @@ ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __rest
         const double d = (double)ds[j];
         const double wj = invW / (d * d);
         const double yc = (double)ys[j] - ybar;
-        rowh[q] = (T)(wj * yc);
         yy += wj * yc * yc;
-        if (write_w) {
+        if (dy_per_series) {
+            rowh[q] = (T)(wj * yc);
             roww1[q] = (T)wj;
             const double d2 = (double)ds[perm2[q]];
             roww2[q] = (T)(invW / (d2 * d2));
+        } else {
+            rowh[q] = (T)yc;
         }
     }
     yy = block_sum(yy, red);
@@ -389,14 +390,13 @@ static cudaError_t premultiply_t(ls_plan_s* p, const double* t, const void* y, c
     const int nb = point_blocks(p->Nd, 1);
     PointSet& a = p->ps[0];
     PointSet& b = p->ps[1];
-    if (p->batch == 1)
-        ls_premultiply_kernel<T, true><<<nb, kPreThreads, 0, s>>>(
-            t, (const T*)y, (const T*)dy, p->sums, p->Nd, p->ndf, p->fc, (int)p->n, p->w, a.hist, b.hist, a.perm,
-            b.perm, (R*)a.rec, (R*)b.rec, (T*)a.rows, (T*)b.rows);
-    else
-        ls_premultiply_kernel<T, false><<<nb, kPreThreads, 0, s>>>(
-            t, (const T*)y, (const T*)dy, p->sums, p->Nd, p->ndf, p->fc, (int)p->n, p->w, a.hist, b.hist, a.perm,
-            b.perm, (R*)a.rec, (R*)b.rec, (T*)a.rows, (T*)b.rows);
+#define LS_PREMUL_ARGS                                                                                              \
+    t, (const T*)y, (const T*)dy, p->sums, p->Nd, p->ndf, p->fc, (int)p->n, p->w, a.hist, b.hist, a.perm, b.perm,   \
+        (R*)a.rec, (R*)b.rec, (T*)a.rows, (T*)b.rows
+    if (p->opts.dy_per_series) ls_premultiply_kernel<T, false, false><<<nb, kPreThreads, 0, s>>>(LS_PREMUL_ARGS);
+    else if (p->batch == 1) ls_premultiply_kernel<T, true, true><<<nb, kPreThreads, 0, s>>>(LS_PREMUL_ARGS);
+    else ls_premultiply_kernel<T, false, true><<<nb, kPreThreads, 0, s>>>(LS_PREMUL_ARGS);
+#undef LS_PREMUL_ARGS
     return cudaGetLastError();
 }
 

@@ -47,7 +47,8 @@ template <typename T>
 struct SpreadSeg {
     const int* bin_start;
     const typename RecOf<T>::type* rec;
-    const T* rows;                   // first row of this segment
+    const T* rows;                   // stored strength rows of this point set (physical row 0)
+    int first_row;                   // logical index of the launch's first row within the point set
     typename V2<T>::type* grid;      // first slot of this segment, [nrows][n]
     int nrows, ngroups;
 };
@@ -64,6 +65,8 @@ struct SpreadArgs {
     int fft_rb;                      // pass-1 radix / 16: row = fft_rb * i + j
     const int* tile_list;            // own FFT: [2][ntiles] tiles that hold points, per point set (x2, x1)
     const int* tile_counts;          // own FFT: [2] lengths of the two lists
+    int w_implicit;                  // shared dy: logical row 0 (the w transform) has strength 1 (the weights are
+                                     // folded into the records' phasors) and is not stored; stored row = logical - 1
     long long Nd;
     SpreadSeg<T> seg[2];             // blockIdx.y < seg[0].ngroups: x2 rows, else x1 rows
     T c[kHalfMax][kMaxDeg + 1];      // only degrees <= PolyDeg<T> are read
@@ -352,7 +355,10 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
                 // strengths are fetched with the record, not after it: one global round trip, not two
 #pragma unroll
                 for (int s = 0; s < NS; ++s)
-                    if (s < nr) r[s] = __ldg(&sg.rows[(long long)(row0 + s) * a.Nd + g]);
+                    if (s < nr) {
+                        const int lr = sg.first_row + row0 + s;
+                        r[s] = (a.w_implicit && lr == 0) ? (T)1 : __ldg(&sg.rows[(long long)(lr - a.w_implicit) * a.Nd + g]);
+                    }
                 rel = l0 + shift - tile_lo;          // first touched cell, tile-relative
                 have = rel + w > 0 && rel < Lt;
             }
@@ -475,6 +481,7 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.skip_empty = p->own_fft ? 1 : 0;
     a.row_masks = p->row_masks;
     a.tile_list = p->tile_list;
+    a.w_implicit = p->opts.dy_per_series ? 0 : 1;
     a.tile_counts = p->tile_counts;
     a.ncoltiles = std::max(1, 65536 / p->L);
     a.fft_rb = p->own_fft ? own_fft_rb(p) : 1;
@@ -488,7 +495,8 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
         const PointSet& ps = p->ps[g == 0 ? 1 : 0];
         a.seg[g].bin_start = ps.bin_start;
         a.seg[g].rec = (const R*)ps.rec;
-        a.seg[g].rows = (const T*)ps.rows + (long long)row0[g] * p->Nd;
+        a.seg[g].rows = (const T*)ps.rows;
+        a.seg[g].first_row = row0[g];
         a.seg[g].grid = (T2*)p->grids + (long long)slot0[g] * p->n;
         a.seg[g].nrows = nrows[g];
         a.seg[g].ngroups = (nrows[g] + NS - 1) / NS;
