@@ -156,6 +156,17 @@ int ls_get_launch_counts(ls_plan_t plan, int* own_kernels, int* fft_execs);
 int ls_debug_modes(ls_plan_t plan, int series, int64_t K, const int64_t* kidx, double* out);
 int ls_debug_stats(ls_plan_t plan, double* out);
 
+/* ls_direct_power — verification path, NOT part of ls_execute: the six sums of
+ * Eq. 1 evaluated by brute force, O(Nd K), for the K consecutive frequencies
+ * f0 + (k0 + i) df, i = 0..K-1, of ONE fp64 series, then the same power assembly.  The kind of direct
+ * evaluator the paper measures its errors against and compares with; it lets
+ * the NUFFT path be checked on frequency ranges the CPU oracle cannot cover.
+ *   t, y, dy  device, const double[Nd];   power  device, double[K] (written).
+ * Allocates 40 Nd bytes of scratch, enqueues on `cuda_stream` and SYNCHRONISES it before returning.
+ * Errors: LS_ERR_INVALID_VALUE, LS_ERR_ALLOC, LS_ERR_CUDA. */
+int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                    const void* dy, void* power, void* cuda_stream);
+
 const char* ls_strerror(int code);
 
 /* Frees everything the plan allocated.  NULL is accepted. */

@@ -14,7 +14,7 @@ import os
 __all__ = [
     "LS_F32", "LS_F64", "LS_OK", "STAGES", "LsError", "ls_opts", "lib_path", "load",
     "ls_plan", "ls_execute", "ls_execute_host", "ls_destroy", "ls_get_info", "ls_workspace_bytes", "ls_set_workspace",
-    "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_strerror",
+    "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_strerror", "ls_direct_power",
     "exported_symbols", "Plan",
 ]
 
@@ -64,6 +64,7 @@ _SIGNATURES = {
     "ls_get_launch_counts": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "ls_debug_modes": (C.c_int, [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]),
     "ls_debug_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
+    "ls_direct_power": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
     "ls_strerror": (C.c_char_p, [C.c_int]),
     "ls_destroy": (C.c_int, [C.c_void_p]),
 }
@@ -156,6 +157,14 @@ def ls_set_workspace(plan, buf, nbytes: int) -> None:
     rc = load().ls_set_workspace(plan, C.c_void_p(_ptr(buf)), C.c_size_t(int(nbytes)))
     if rc != LS_OK:
         raise LsError(rc, "ls_set_workspace")
+
+
+def ls_direct_power(Nd, f0, df, k0, K, t, y, dy, power, stream=0) -> None:
+    """Brute-force power of frequencies f0 + (k0 .. k0+K-1) df of one fp64 series (device buffers)."""
+    rc = load().ls_direct_power(int(Nd), float(f0), float(df), int(k0), int(K), C.c_void_p(_ptr(t)), C.c_void_p(_ptr(y)),
+                                C.c_void_p(_ptr(dy)), C.c_void_p(_ptr(power)), C.c_void_p(int(stream)))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_direct_power")
 
 
 def ls_get_stage_ms(plan) -> dict:

@@ -1,0 +1,155 @@
+// ls_direct.cu — brute-force O(N_d K) Lomb-Scargle on the GPU (the style of
+// evaluator the paper compares against, and the definition it measures errors against,
+// PAPER.md:75 "exact angle-sum trigonometric identities ... a 'phase winding' method").
+//
+// Eq. 1 evaluated directly for K consecutive frequencies f_k = f0 + k df of ONE fp64
+// series: the six sums Sh, Ch, S, C, S2, C2, then the same tau / CC, SS / power arithmetic as the NUFFT
+// path (ls_power.cuh).  It exists to verify the NUFFT path on frequency ranges the CPU oracle cannot
+// cover (1e6 frequencies of config 3 take ~2 s here, hours on the host) and is itself parity-tested
+// against the oracle on configs 1-2.  Not part of ls_execute.
+//
+// One thread owns kR consecutive frequencies: per point it seeds e^{2 pi i f t_j} at its first frequency
+// (phase by an FMA two-product of the double-double frequency, one sincospi) and winds it kR - 1 times by
+// the point's step phasor e^{2 pi i df t_j} (computed once per point by a preparation kernel).
+#include "ls_internal.h"
+#include "ls_power.cuh"
+
+namespace lsb {
+namespace {
+
+constexpr int kDirThreads = 128;
+constexpr int kR = 8;                      // frequencies per thread
+constexpr int kTilePts = 512;              // points staged in shared memory per pass
+
+struct DirPoint {                          // per point, written by the preparation kernel
+    double t, w, h, cd, sd;                // time, w_j, h_j = w_j (y_j - ybar), step phasor e^{2 pi i df t_j}
+};
+
+__device__ __forceinline__ double warp_sum_d(double v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// sums[0] += sum dy^-2, sums[1] += sum dy^-2 y
+__global__ void ls_direct_stats_kernel(const double* __restrict__ y, const double* __restrict__ dy, long long Nd,
+                                       double* __restrict__ sums) {
+    double a = 0.0, b = 0.0;
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < Nd; j += (long long)gridDim.x * blockDim.x) {
+        const double iv = 1.0 / (dy[j] * dy[j]);
+        a += iv;
+        b += iv * y[j];
+    }
+    a = warp_sum_d(a);
+    b = warp_sum_d(b);
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(&sums[0], a);
+        atomicAdd(&sums[1], b);
+    }
+}
+
+// per point: normalised weight, centred strength, step phasor; sums[2] += YY
+__global__ void ls_direct_prepare_kernel(const double* __restrict__ t, const double* __restrict__ y,
+                                         const double* __restrict__ dy, long long Nd, double df, double* __restrict__ sums,
+                                         DirPoint* __restrict__ pts) {
+    const double W = sums[0], ybar = sums[1] / W;
+    double yy = 0.0;
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < Nd; j += (long long)gridDim.x * blockDim.x) {
+        DirPoint p;
+        p.t = t[j];
+        p.w = 1.0 / (dy[j] * dy[j]) / W;
+        const double yc = y[j] - ybar;
+        p.h = p.w * yc;
+        yy += p.w * yc * yc;
+        const double pr = df * p.t, er = fma(df, p.t, -pr);      // df t = pr + er exactly
+        double ph = (pr - rint(pr)) + er;
+        ph -= rint(ph);
+        sincospi(2.0 * ph, &p.sd, &p.cd);
+        pts[j] = p;
+    }
+    yy = warp_sum_d(yy);
+    if ((threadIdx.x & 31) == 0) atomicAdd(&sums[2], yy);
+}
+
+__global__ void __launch_bounds__(kDirThreads)
+ls_direct_kernel(const DirPoint* __restrict__ pts, long long Nd, double f0, double df, long long k0, long long K,
+                 const double* __restrict__ sums, double* __restrict__ power) {
+    __shared__ DirPoint sp[kTilePts];
+    const long long kfirst = ((long long)blockIdx.x * kDirThreads + threadIdx.x) * kR;   // offset inside [0, K)
+    // f = f0 + (k0 + kfirst) df as a double-double (error-free product + two-sum)
+    const double kd = (double)(k0 + kfirst);
+    const double pk = kd * df, pe = fma(kd, df, -pk);
+    const double fs = f0 + pk, bb = fs - f0;
+    const double se = (f0 - (fs - bb)) + (pk - bb);
+    const double flo0 = se + pe;
+    const double fhi = fs + flo0, flo = flo0 - (fhi - fs);
+
+    double Sh[kR], Ch[kR], S[kR], C[kR], S2[kR], C2[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) Sh[r] = Ch[r] = S[r] = C[r] = S2[r] = C2[r] = 0.0;
+
+    for (long long base = 0; base < Nd; base += kTilePts) {
+        const int cnt = (int)min((long long)kTilePts, Nd - base);
+        __syncthreads();
+        for (int i = threadIdx.x; i < cnt; i += kDirThreads) sp[i] = pts[base + i];
+        __syncthreads();
+        if (kfirst >= K) continue;
+        for (int i = 0; i < cnt; ++i) {
+            const DirPoint p = sp[i];
+            const double pr = fhi * p.t, er = fma(fhi, p.t, -pr) + flo * p.t;
+            double ph = (pr - rint(pr)) + er;
+            ph -= rint(ph);
+            double s, c;
+            sincospi(2.0 * ph, &s, &c);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                Sh[r] = fma(p.h, s, Sh[r]);
+                Ch[r] = fma(p.h, c, Ch[r]);
+                S[r] = fma(p.w, s, S[r]);
+                C[r] = fma(p.w, c, C[r]);
+                S2[r] = fma(p.w, 2.0 * s * c, S2[r]);
+                C2[r] = fma(p.w, fma(-2.0 * s, s, 1.0), C2[r]);
+                const double cn = fma(c, p.cd, -s * p.sd);        // wind to the next frequency
+                s = fma(s, p.cd, c * p.sd);
+                c = cn;
+            }
+        }
+    }
+    if (kfirst >= K) return;
+    const double inv_YY = 1.0 / sums[2];
+#pragma unroll
+    for (int r = 0; r < kR; ++r)
+        if (kfirst + r < K) power[kfirst + r] = series_power(freq_terms(S[r], C[r], S2[r], C2[r]), Sh[r], Ch[r], inv_YY);
+}
+
+}  // namespace
+}  // namespace lsb
+
+extern "C" int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                               const void* dy, void* power, void* cuda_stream) {
+    using namespace lsb;
+    if (Nd < 1 || K < 1 || k0 < 0 || !t || !y || !dy || !power || !(df > 0.0) || !(f0 >= 0.0)) return LS_ERR_INVALID_VALUE;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    double* sums = nullptr;
+    DirPoint* pts = nullptr;
+    if (cudaMalloc((void**)&sums, 4 * sizeof(double)) != cudaSuccess || cudaMalloc((void**)&pts, (size_t)Nd * sizeof(DirPoint)) != cudaSuccess) {
+        cudaGetLastError();
+        cudaFree(sums);
+        return LS_ERR_ALLOC;
+    }
+    int rc = LS_OK;
+    const int nb = (int)std::min<long long>((Nd + 255) / 256, 1184);
+    if (cudaMemsetAsync(sums, 0, 4 * sizeof(double), s) != cudaSuccess) rc = LS_ERR_CUDA;
+    if (rc == LS_OK) {
+        ls_direct_stats_kernel<<<nb, 256, 0, s>>>((const double*)y, (const double*)dy, Nd, sums);
+        ls_direct_prepare_kernel<<<nb, 256, 0, s>>>((const double*)t, (const double*)y, (const double*)dy, Nd, df, sums, pts);
+        const long long threads = (K + kR - 1) / kR;
+        ls_direct_kernel<<<(unsigned)((threads + kDirThreads - 1) / kDirThreads), kDirThreads, 0, s>>>(
+            pts, Nd, f0, df, k0, K, sums, (double*)power);
+        if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) rc = LS_ERR_CUDA;
+    }
+    cudaFree(sums);
+    cudaFree(pts);
+    if (rc != LS_OK) cudaGetLastError();
+    return rc;
+}

@@ -1,0 +1,76 @@
+"""-m gpu tests of the brute-force GPU evaluator (ls_direct_power) and, through it, of the NUFFT
+path on frequency ranges the CPU oracle cannot cover.
+
+1. ls_direct_power against the CPU oracle (configs 1 and 2): it is a verification tool, so it is itself checked first.
+2. ls_execute (own FFT, fused) against ls_direct_power on 1.3 million frequencies of config 3 — contiguous slabs at
+   both ends of the grid, across the mode-wrap seam and around the injected peak — where the oracle can only sample."""
+import numpy as np
+import pytest
+
+from gpu_util import GATE_F64, errors, gpu_power, oracle_power, require_cuda
+from paper_2409_08090_b200.workloads import make_workload
+
+pytestmark = pytest.mark.gpu
+
+
+def _direct(w, k0, K):
+    torch = require_cuda()
+    from paper_2409_08090_b200 import binding as B
+    dev = torch.device("cuda:0")
+    t = torch.from_numpy(w.t).to(dev); y = torch.from_numpy(np.ascontiguousarray(w.y[0])).to(dev)
+    dy = torch.from_numpy(w.dy).to(dev)
+    P = torch.full((K,), float("nan"), dtype=torch.float64, device=dev)
+    B.ls_direct_power(w.Nd, w.f0, w.df, k0, K, t, y, dy, P, torch.cuda.current_stream().cuda_stream)
+    return P.cpu().numpy()
+
+
+def test_direct_against_oracle_cfg1_full_grid():
+    w = make_workload(1)
+    Pd = _direct(w, 0, w.Nf)
+    Po = oracle_power(w)
+    e = errors(Pd, Po)
+    assert e["Einf"] <= 1e-12 and e["max"] <= 1e-9, e          # direct vs direct: rounding only
+
+
+def test_direct_against_oracle_cfg2_offset_range_and_ragged_tail():
+    w = make_workload(2)
+    k0, K = 100_003, 24_997                                     # not a multiple of the 8 frequencies per thread
+    Pd = _direct(w, k0, K)
+    Po = oracle_power(w, fast=True)[k0:k0 + K]
+    e = errors(Pd, Po)
+    assert e["Einf"] <= 1e-12 and e["max"] <= 1e-8, e
+    ks = np.arange(k0, k0 + K, 97)
+    assert np.max(np.abs(Pd[ks - k0] - oracle_power(w, ks=ks))) <= 1e-12
+
+
+def test_direct_rejects_bad_arguments():
+    require_cuda()
+    from paper_2409_08090_b200 import binding as B
+    with pytest.raises(B.LsError):
+        B.ls_direct_power(0, 0.1, 0.1, 0, 10, 1, 1, 1, 1)
+    with pytest.raises(B.LsError):
+        B.ls_direct_power(10, 0.1, 0.0, 0, 10, 1, 1, 1, 1)
+    with pytest.raises(B.LsError):
+        B.ls_direct_power(10, 0.1, 0.1, 0, 10, 0, 1, 1, 1)      # NULL t
+
+
+def test_cfg3_nufft_path_against_direct_on_wide_ranges():
+    """Headline size, launch configuration of bench.py (auto plan: n = 2^24, own FFT, fused last pass)."""
+    w = make_workload(3)
+    Pg = gpu_power(w)[0]
+    half = w.Nf // 2
+    kpk = int(round((1 / 1.7 - w.f0) / w.df))
+    slabs = [(0, 1 << 18), (half - (1 << 17), 1 << 18), (w.Nf - (1 << 18), 1 << 18), (3_000_000, 1 << 18),
+             (9_000_001, (1 << 18) + 5)]                      # the first slab holds the injected peak (k ~ 29 400)
+    assert 0 <= kpk < (1 << 18)
+    pmax = Pg.max()
+    worst, rel = 0.0, []
+    for k0, K in slabs:
+        Pd = _direct(w, k0, K)
+        d = np.abs(Pg[k0:k0 + K] - Pd)
+        worst = max(worst, float(d.max()))
+        rel.append(d / np.maximum(Pd, 1e-300))
+    rel = np.concatenate(rel)
+    assert worst / pmax <= GATE_F64, worst / pmax
+    assert np.median(rel) <= 1e-8 and np.percentile(rel, 99) <= 1e-6, (np.median(rel), np.percentile(rel, 99))
+    assert int(np.argmax(Pg)) == kpk or abs(int(np.argmax(Pg)) - kpk) <= 1
