@@ -74,3 +74,23 @@ def test_cfg3_nufft_path_against_direct_on_wide_ranges():
     assert worst / pmax <= GATE_F64, worst / pmax
     assert np.median(rel) <= 1e-8 and np.percentile(rel, 99) <= 1e-6, (np.median(rel), np.percentile(rel, 99))
     assert int(np.argmax(Pg)) == kpk or abs(int(np.argmax(Pg)) - kpk) <= 1
+
+
+def test_cfg5_fp32_path_against_direct_on_ranges():
+    """Config 5 at full size (fp32 grids, autotuned n): three slabs of 2^15 frequencies against the fp64 brute force
+    evaluated on the same (exactly promoted) fp32 inputs; gate of the fp32 config (north_star: <= 1e-4)."""
+    from gpu_util import GATE_F32
+    w = make_workload(5)
+    Pg = gpu_power(w)[0]
+    w64 = type(w)(w.name, w.t, w.y.astype(np.float64), w.dy.astype(np.float64), w.f0, w.df, w.Nf, "f64", w.eps)
+    kpk = int(round((1 / 0.9137 - w.f0) / w.df))
+    pmax = float(Pg.max())
+    worst, rel = 0.0, []
+    for k0 in (0, max(0, kpk - (1 << 14)), w.Nf // 2 - (1 << 14), w.Nf - (1 << 15)):
+        Pd = _direct(w64, k0, 1 << 15)
+        d = np.abs(Pg[k0:k0 + (1 << 15)] - Pd)
+        worst = max(worst, float(d.max()))
+        rel.append(d / np.maximum(Pd, 1e-300))
+    rel = np.concatenate(rel)
+    assert worst / pmax <= GATE_F32, worst / pmax
+    assert np.median(rel) <= 1e-4, np.median(rel)
