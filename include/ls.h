@@ -45,6 +45,7 @@ extern "C" {
 
 typedef struct ls_plan_s* ls_plan_t;            /* opaque; owns cuFFT plan, tables, scratch */
 
+enum { LS_NORM_STANDARD = 0, LS_NORM_MODEL = 1, LS_NORM_LOG = 2, LS_NORM_PSD = 3 };
 enum { LS_F32 = 0, LS_F64 = 1 };                /* dtype of y, dy, power, fine grid and FFT (A9:
                                                    t, grid coordinates, phase reduction and the
                                                    assembly are fp64 for both) */
@@ -92,7 +93,11 @@ typedef struct {
     int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs an
                                fp64 grid of 2^20..2^24 cells; LS_ERR_UNSUPPORTED otherwise), 3 = as 2 but with
                                deconvolution + assembly as a separate kernel (clean stage timings)  */
-    int reserved[5];        /* must be zero                                                       */
+    int no_floating_mean;   /* 0: floating mean, six sums (default; north_star).  1: the fixed-mean form of
+                               PAPER.md:17 ("four weighted trigonometric sums"): y centred by its weighted
+                               mean, sinusoid model without an offset term                          */
+    int normalization;      /* LS_NORM_STANDARD (default), _MODEL, _LOG, _PSD            */
+    int reserved[3];        /* must be zero                                                       */
 } ls_opts;
 
 /* ls_plan — choose (sigma, w, beta, n) from eps ("width and fine grid size are

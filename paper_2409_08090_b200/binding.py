@@ -20,6 +20,7 @@ __all__ = [
 
 LS_F32, LS_F64 = 0, 1
 LS_OK = 0
+LS_NORM_STANDARD, LS_NORM_MODEL, LS_NORM_LOG, LS_NORM_PSD = 0, 1, 2, 3
 STAGES = ("stats", "sort", "premul", "spread", "fft", "assemble", "total", "fft_pass1", "fft_pass2", "fft_pass3")
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
@@ -38,7 +39,9 @@ class ls_opts(C.Structure):
         ("no_autotune", C.c_int),
         ("graph", C.c_int),
         ("fft_impl", C.c_int),
-        ("reserved", C.c_int * 5),
+        ("no_floating_mean", C.c_int),
+        ("normalization", C.c_int),
+        ("reserved", C.c_int * 3),
     ]
 
 

@@ -340,7 +340,9 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
                               o.tile_cells > lsb::kSpreadThreads * 4))
         return LS_ERR_INVALID_VALUE;
-    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 3) return LS_ERR_INVALID_VALUE;
+    if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 3 ||
+        o.no_floating_mean < 0 || o.no_floating_mean > 1 || o.normalization < 0 || o.normalization > 3)
+        return LS_ERR_INVALID_VALUE;
 
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || o.device < 0 || o.device >= ndev) return LS_ERR_CUDA;

@@ -124,6 +124,7 @@ struct FftArgs {
     const double* sums;        // [batch][4]: YY at [4 s + 2]
     double* power;             // [batch][Nf]
     int series0;
+    int no_float, norm;        // opts.no_floating_mean, opts.normalization
 };
 
 __device__ __forceinline__ double2 twiddle_n(const FftArgs& a, unsigned e) {
@@ -281,7 +282,8 @@ ls_fft_rows_kernel(const FftArgs a) {
         const long long kk0 = (long long)(k1b + c) + (long long)a.R1 * k2;
         const long long r12 = (long long)a.R1 * a.R2;
         const int ser = a.series0 + tr;
-        const double inv_YY = FUSED ? 1.0 / a.sums[4 * ser + 2] : 0.0;
+        const double YYs = FUSED ? a.sums[4 * ser + 2] : 1.0;
+        const double inv_YY = 1.0 / YYs;
         if (FUSED) {
             // K5: diagonal rescaling of the three modes of frequency k; K6: tau rotation and power.  Four
             // frequencies at a time: their 12 loads are in flight together before any arithmetic starts.
@@ -307,8 +309,10 @@ ls_fft_rows_kernel(const FftArgs a) {
                 for (int q = 0; q < 4; ++q) {
                     if (k[q] < a.Nf) {
                         const double2 gh = x[pos16(g + q)];
-                        const FreqTerms f = freq_terms(gw[q].y * d[q], gw[q].x * d[q], g2[q].y * d[q], g2[q].x * d[q]);
-                        a.power[(long long)ser * a.Nf + k[q]] = series_power(f, gh.y * d[q], gh.x * d[q], inv_YY);
+                        const double dw = a.no_float ? 0.0 : d[q];       // fixed mean: S = C = 0
+                        const FreqTerms f = freq_terms(gw[q].y * dw, gw[q].x * dw, g2[q].y * d[q], g2[q].x * d[q]);
+                        const double P = series_power(f, gh.y * d[q], gh.x * d[q], inv_YY);
+                        a.power[(long long)ser * a.Nf + k[q]] = apply_normalization(P, a.norm, YYs, a.sums[0]);
                     }
                 }
             }
@@ -385,6 +389,8 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.sums = p->sums;
     a.power = nullptr;
     a.series0 = 0;
+    a.no_float = p->opts.no_floating_mean;
+    a.norm = p->opts.normalization;
 }
 
 // Pass 1 of transforms [slot0, slot0 + ntrans) of the plan's grids; the first n_x2 of them belong to the x2

@@ -47,6 +47,8 @@ struct AssembleArgs {
     long long n, Nf;
     long long stride;               // elements between transforms: n, or Nf when compact
     int compact;                    // 1: mode k of a transform sits at index k
+    int no_float;                   // opts.no_floating_mean: the (S, C) sums of the weights drop out
+    int norm;                       // opts.normalization
     long long half;                 // floor(Nf/2)
     const double* dinv;
     const double* sums;
@@ -70,10 +72,11 @@ ls_assemble_kernel(const AssembleArgs a) {
     const T2 gh = __ldcs(&g[(long long)(a.h_slot + i * a.h_stride) * a.stride + idx]);
     const T2 gw = g[(long long)(a.w_slot + i * a.w_stride) * a.stride + idx];
     const T2 g2 = g[(long long)(a.w2_slot + i * a.w2_stride) * a.stride + idx];
-    const double YY = a.sums[4 * s + 2];
-    const double P = assemble_power((double)gh.y * d, (double)gh.x * d, (double)gw.y * d, (double)gw.x * d,
+    const double YY = a.sums[4 * s + 2], W = a.sums[a.dy_per_series ? 4 * s : 0];
+    const double dw = a.no_float ? 0.0 : d;        // fixed mean: S = C = 0
+    const double P = assemble_power((double)gh.y * d, (double)gh.x * d, (double)gw.y * dw, (double)gw.x * dw,
                                     (double)g2.y * d, (double)g2.x * d, 1.0 / YY);
-    reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k] = (T)P;
+    reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k] = (T)apply_normalization(P, a.norm, YY, W);
 }
 
 // Batch with shared dy: the (w, w2) transforms and hence FreqTerms are common to all series, so one
@@ -91,15 +94,18 @@ ls_assemble_shared_kernel(const AssembleArgs a, int nseries) {
     const T2* g = reinterpret_cast<const T2*>(a.grids);
     const T2 gw = g[(long long)a.w_slot * a.stride + idx];
     const T2 g2 = g[(long long)a.w2_slot * a.stride + idx];
-    const FreqTerms f = freq_terms((double)gw.y * d, (double)gw.x * d, (double)g2.y * d, (double)g2.x * d);
+    const double dw = a.no_float ? 0.0 : d;        // fixed mean: S = C = 0
+    const FreqTerms f = freq_terms((double)gw.y * dw, (double)gw.x * dw, (double)g2.y * d, (double)g2.x * d);
+    const double W = a.sums[0];
     const int i0 = blockIdx.y * kSeriesPerThread;
     const int i1 = min(i0 + kSeriesPerThread, nseries);
 #pragma unroll 4
     for (int i = i0; i < i1; ++i) {
         const int s = a.series0 + i;
         const T2 gh = __ldcs(&g[(long long)(a.h_slot + i) * a.stride + idx]);
-        const double P = series_power(f, (double)gh.y * d, (double)gh.x * d, 1.0 / a.sums[4 * s + 2]);
-        __stcs(&reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k], (T)P);
+        const double YY = a.sums[4 * s + 2];
+        const double P = series_power(f, (double)gh.y * d, (double)gh.x * d, 1.0 / YY);
+        __stcs(&reinterpret_cast<T*>(a.power)[(long long)s * a.Nf + k], (T)apply_normalization(P, a.norm, YY, W));
     }
 }
 
@@ -139,6 +145,8 @@ cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, 
     a.Nf = p->Nf;
     a.stride = p->own_fft ? p->Nf : p->n;
     a.compact = p->own_fft ? 1 : 0;
+    a.no_float = p->opts.no_floating_mean;
+    a.norm = p->opts.normalization;
     a.half = p->Nf / 2;
     a.dinv = p->dinv;
     a.sums = p->sums;

@@ -2,6 +2,8 @@
 // with the assembly (ls_fft.cu).  Device-only, header-only; internal to libls_b200.so.
 #pragma once
 
+#include "../../include/ls.h"
+
 namespace lsb {
 
 // The assembly formulas exactly as north_star lists them, with
@@ -48,6 +50,15 @@ __device__ __forceinline__ double series_power(const FreqTerms& f, double Sh, do
     const double YC = Ch * f.Cw + Sh * f.Sw;
     const double YS = Sh * f.Cw - Ch * f.Sw;
     return (YC * YC * f.iCC + YS * YS * f.iSS) * inv_YY;
+}
+// Normalisations of the standard power P = 1 - chi2/chi2_ref (VanderPlas 2018, cited PAPER.md:117; the
+// Astropy interface the paper plugs into): model P/(1-P), log -ln(1-P), psd P W YY / 2
+// (W = sum dy^-2, YY = weighted variance: W YY = chi2_ref).
+__device__ __forceinline__ double apply_normalization(double P, int norm, double YY, double W) {
+    if (norm == LS_NORM_MODEL) return P / (1.0 - P);
+    if (norm == LS_NORM_LOG) return -log(1.0 - P);
+    if (norm == LS_NORM_PSD) return 0.5 * P * W * YY;
+    return P;
 }
 __device__ __forceinline__ double assemble_power(double Sh, double Ch, double S, double C, double S2, double C2,
                                                  double inv_YY) {

@@ -46,7 +46,9 @@ def test_ls_opts_layout_matches_header():
     assert ls_opts.no_autotune.offset == 36
     assert ls_opts.graph.offset == 40
     assert ls_opts.fft_impl.offset == 44
-    assert ls_opts.reserved.offset == 48
+    assert ls_opts.no_floating_mean.offset == 48
+    assert ls_opts.normalization.offset == 52
+    assert ls_opts.reserved.offset == 56
     assert ctypes.sizeof(ls_opts) == 72
 
 

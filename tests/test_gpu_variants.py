@@ -1,0 +1,53 @@
+"""-m gpu parity of the periodogram variants (fixed mean = the "four sums" of PAPER.md:17, and the
+normalisations of the Astropy interface) against oracle/variants.py, on the cuFFT path, on the own-FFT
+path with the fused last pass, and for a batch."""
+import numpy as np
+import pytest
+
+from gpu_util import gpu_power
+from oracle import variants
+from paper_2409_08090_b200.workloads import Workload, compare_indices, scaled_workload
+
+pytestmark = pytest.mark.gpu
+NORM = {"standard": 0, "model": 1, "log": 2, "psd": 3}
+
+
+def _rel(Pg, Po):
+    return float(np.max(np.abs(Pg - Po)) / np.max(np.abs(Po)))
+
+
+@pytest.mark.parametrize("fit_mean", [True, False])
+@pytest.mark.parametrize("norm", ["standard", "model", "log", "psd"])
+def test_variants_small_grid_cufft_path(fit_mean, norm):
+    w = scaled_workload(2, 3000)
+    Pg = gpu_power(w, no_floating_mean=0 if fit_mean else 1, normalization=NORM[norm])[0]
+    Po = variants.power(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, fit_mean=fit_mean, normalization=norm)
+    assert _rel(Pg, Po) <= 1e-8, (fit_mean, norm, _rel(Pg, Po))
+
+
+@pytest.mark.parametrize("fit_mean,norm", [(False, "standard"), (False, "psd"), (True, "log")])
+def test_variants_own_fft_fused_path(fit_mean, norm):
+    rng = np.random.default_rng(90)
+    Nf = int(0.7 * (1 << 20)); Nd = Nf // 12
+    t = rng.uniform(0, 800.0, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    y = 5.0 + np.sin(2 * np.pi * (df + 40000 * df) * t) + rng.normal(0, 1.0, Nd)
+    w = Workload("variants_p20", t, np.ascontiguousarray(y[None]), dy, df, df, Nf, "f64", 1e-9)
+    Pg, ex = gpu_power(w, no_autotune=1, no_floating_mean=0 if fit_mean else 1, normalization=NORM[norm],
+                       return_plan_info=True)
+    assert ex["launches"][1] == 0                                   # own FFT, no cuFFT exec
+    ks = np.unique(np.concatenate([compare_indices(w, 300), np.arange(39995, 40006)]))
+    Po = variants.power(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, k=ks, fit_mean=fit_mean, normalization=norm)
+    assert _rel(Pg[0][ks], Po) <= 1e-8
+
+
+def test_variants_batch_shared_and_per_series_dy():
+    w = scaled_workload(4, 1500, batch=6)
+    for per in (False, True):
+        if per:
+            w.dy = np.ascontiguousarray(np.random.default_rng(5).uniform(0.5, 1.5, (6, w.Nd)))
+        Pg = gpu_power(w, no_floating_mean=1, normalization=NORM["model"])
+        for b in (0, 5):
+            dyb = w.dy[b] if per else w.dy
+            Po = variants.power(w.t, w.y[b], dyb, w.f0, w.df, w.Nf, fit_mean=False, normalization="model")
+            assert _rel(Pg[b], Po) <= 1e-8, (per, b)
