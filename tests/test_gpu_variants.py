@@ -51,3 +51,25 @@ def test_variants_batch_shared_and_per_series_dy():
             dyb = w.dy[b] if per else w.dy
             Po = variants.power(w.t, w.y[b], dyb, w.f0, w.df, w.Nf, fit_mean=False, normalization="model")
             assert _rel(Pg[b], Po) <= 1e-8, (per, b)
+
+
+def test_astropy_style_front_end():
+    import torch
+    from paper_2409_08090_b200.lombscargle import LombScargle
+    w = scaled_workload(2, 2000)
+    ls = LombScargle(w.t, w.y[0], w.dy, fit_mean=False, normalization="psd")
+    f0, df, Nf = ls.autofrequency(samples_per_peak=5, nyquist_factor=3)
+    T = w.t.max() - w.t.min()
+    assert df == pytest.approx(1 / (5 * T)) and f0 == pytest.approx(df / 2) and Nf > 1000
+    freq, P = ls.autopower(samples_per_peak=5, nyquist_factor=3)
+    torch.cuda.synchronize()
+    assert P.shape == (Nf,) and freq.shape == (Nf,) and float(freq[1] - freq[0]) == pytest.approx(df)
+    Po = variants.power(w.t, w.y[0], w.dy, f0, df, Nf, fit_mean=False, normalization="psd")
+    assert _rel(P.cpu().numpy(), Po) <= 1e-8
+    P2 = ls.power_grid(w.f0, w.df, w.Nf)                           # explicit grid, replaces the cached plan
+    torch.cuda.synchronize()
+    assert _rel(P2.cpu().numpy(), variants.power(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, fit_mean=False,
+                                                 normalization="psd")) <= 1e-8
+    ls.close()
+    with pytest.raises(ValueError):
+        LombScargle(w.t, w.y[0], w.dy, normalization="nope")
