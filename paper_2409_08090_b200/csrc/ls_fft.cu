@@ -252,7 +252,9 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
 // Pass 3: the transform dimension (l3) is contiguous; the CTA takes 16 consecutive k1 at one k2, so that the
 // kept modes leave in runs of 16 consecutive frequencies.  Output: modes[tr][k], k = (kk + half) mod n < Nf,
 // kk = k1 + R1 k2 + R1 R2 k3 the stored mode index (= k' mod n).
-template <bool FUSED>
+// VARIANT: opts.no_floating_mean / opts.normalization in effect (kept out of the default instantiation: the extra
+// branches cost the fused kernel 20 us at config 3).
+template <bool FUSED, bool VARIANT = false>
 __global__ void __launch_bounds__(kFftThreads, 512 / kFftThreads)
 ls_fft_rows_kernel(const FftArgs a) {
     extern __shared__ __align__(16) unsigned char fsm[];
@@ -309,10 +311,11 @@ ls_fft_rows_kernel(const FftArgs a) {
                 for (int q = 0; q < 4; ++q) {
                     if (k[q] < a.Nf) {
                         const double2 gh = x[pos16(g + q)];
-                        const double dw = a.no_float ? 0.0 : d[q];       // fixed mean: S = C = 0
+                        const double dw = (VARIANT && a.no_float) ? 0.0 : d[q];       // fixed mean: S = C = 0
                         const FreqTerms f = freq_terms(gw[q].y * dw, gw[q].x * dw, g2[q].y * d[q], g2[q].x * d[q]);
-                        const double P = series_power(f, gh.y * d[q], gh.x * d[q], inv_YY);
-                        a.power[(long long)ser * a.Nf + k[q]] = apply_normalization(P, a.norm, YYs, a.sums[0]);
+                        double P = series_power(f, gh.y * d[q], gh.x * d[q], inv_YY);
+                        if (VARIANT) P = apply_normalization(P, a.norm, YYs, a.sums[0]);
+                        a.power[(long long)ser * a.Nf + k[q]] = P;
                     }
                 }
             }
@@ -366,6 +369,7 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(ls_fft_rows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem);
 }
 
@@ -441,7 +445,8 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
     a.power = (double*)power;
     a.series0 = series0;
     dim3 g3(a.R1 / kC, 256, nseries);
-    ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
+    if (a.no_float || a.norm) ls_fft_rows_kernel<true, true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
+    else ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
 
