@@ -13,12 +13,14 @@
  *   which are the real/imaginary parts of three type-1 (non-uniform -> uniform) NUFFTs
  *   (PAPER.md:24-27 Eq. 2, :45): strengths pre-multiplied by e^{2 pi i f_c t_j}
  *   (f_c = f0 + floor(Nf/2) df; A4), spread onto a fine grid of n ~ sigma Nf cells with the
- *   "exponential of semicircle" kernel, one equispaced FFT (cuFFT), diagonal
- *   rescaling, then the tau / YY,YC,YS,CC,SS assembly named by north_star.
+ *   "exponential of semicircle" kernel, one equispaced FFT, diagonal rescaling
+ *   (PAPER.md:47), then the tau / YY,YC,YS,CC,SS assembly named by north_star.
  *
  * Every step runs in hand-written sm_100a kernels (stats, bin-count + scan, premultiply-scatter,
- * tile-owner spread, deconvolve + assemble) around one cuFFT plan.  There is NO CPU fallback:
- * every entry point fails with LS_ERR_CUDA when no device is usable.
+ * tile-owner spread, deconvolve + assemble).  The fine-grid FFT is the library's own three-pass
+ * transform for fp64 grids of 2^20..2^24 cells (pruned first pass, last pass fused with the
+ * assembly) and one cuFFT plan for every other grid.  There is NO CPU fallback: every entry point
+ * fails with LS_ERR_CUDA when no device is usable.
  *
  * Conventions
  *   - All functions return an int status (LS_OK == 0); nothing throws, prints or exits.
