@@ -172,6 +172,7 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
         for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * kC + c];
         fft16(x);
         // k_r = ka + 16 kb;  twiddle exponent e = k_r * m * outer (mod n) = e0 + kb * de
+        // (requesting the tables before the exchange, as pass 1 does, costs this DRAM-bound pass registers: slower)
         const unsigned mm = (unsigned)m * (unsigned)outer;
         double2 tw = twiddle_n(a, (unsigned)ka * mm);
         const double2 st = twiddle_n(a, 16u * mm);
@@ -211,6 +212,10 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
         const int tr = tile / tiles_per_trans;
         const long long m = (long long)(tile - tr * tiles_per_trans) * C + c;
         double2* base = a.grids + (long long)tr * a.n + m;
+        // the table loads of the inter-pass twiddles are requested with the data, not after the exchange
+        const unsigned mm = (unsigned)m;
+        const double2 st = twiddle_n(a, 16u * mm);
+        const double2 tw0 = twiddle_n(a, (unsigned)(hi * NI) * mm);
         {
             const int j = hi;
             double2 x[16];
@@ -227,8 +232,6 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
         }
         __syncthreads();
         {
-            const unsigned mm = (unsigned)m;
-            const double2 st = twiddle_n(a, 16u * mm);
 #pragma unroll
             for (int q = 0; q < NI; ++q) {
                 const int ka = hi * NI + q;
@@ -237,7 +240,7 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
                 for (int j = 0; j < RB; ++j) y[j] = Y[(ka * RB + j) * C + c];
                 fft_small<RB>(y);
                 // k1 = ka + 16 kb;  twiddle exponent k1 * m = ka m + kb (16 m)
-                double2 tw = twiddle_n(a, (unsigned)ka * mm);
+                double2 tw = q == 0 ? tw0 : twiddle_n(a, (unsigned)ka * mm);
 #pragma unroll
                 for (int kb = 0; kb < RB; ++kb) {
                     base[(long long)(ka + 16 * kb) * inner] = cmul(y[fft_pos<RB>(kb)], tw);
