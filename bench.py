@@ -303,7 +303,7 @@ def run_ours(args):
     if not args.upsampfac:
         popts["upsampfac"] = info["n"] / w.Nf * (1 - 1e-12) if info["n"] & (info["n"] - 1) else 0.0   # same n as `plan`
     plan_t = None
-    if popts["fft_impl"] in (0, 2):
+    if popts["fft_impl"] == 2:
         try:
             plan_t = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, ldt, w.batch, timing=1, no_autotune=1,
                             **dict(popts, fft_impl=3))

@@ -70,8 +70,8 @@ enum {
     LS_STAGE_FFT = 4,           /* F   the fine-grid FFT: cuFFT, or the own passes 1-3 (reported
                                        separately, north_star)                                   */
     LS_STAGE_ASSEMBLE = 5,      /* K5+K6 mode extraction, deconvolution, tau + power assembly; with
-                                       the own FFT (fft_impl 0/2) it contains the h transforms'
-                                       third FFT pass, which is fused with it                    */
+                                       fft_impl = 2 it contains the h transforms' third FFT pass,
+                                       which is fused with it                    */
     LS_STAGE_TOTAL = 6,         /* whole execute                                                 */
     LS_STAGE_FFT_PASS1 = 7,     /* own FFT only: the three passes, also summed into LS_STAGE_FFT  */
     LS_STAGE_FFT_PASS2 = 8,
@@ -92,9 +92,11 @@ typedef struct {
     int graph;              /* CUDA-graph replay of the execute sequence (needs timing == 0 and a non-legacy
                                stream): 0 = auto (on; off for good after three consecutive executes
                                with changed buffer pointers), 1 = never, 2 = always                 */
-    int fft_impl;           /* 0 = auto, 1 = cuFFT plan, 2 = the library's own three-pass FFT (needs an
-                               fp64 grid of 2^20..2^24 cells; LS_ERR_UNSUPPORTED otherwise), 3 = as 2 but with
-                               deconvolution + assembly as a separate kernel (clean stage timings)  */
+    int fft_impl;           /* 0 = auto (the library's own three-pass FFT where it exists — fp64 grids of
+                               2^20..2^24 cells — else cuFFT), 1 = cuFFT plan, 2 = own FFT with the h
+                               transforms' last pass fused with deconvolution + assembly, 3 = own FFT
+                               with the assembly as a separate kernel (what auto picks; 2 and 3 give
+                               LS_ERR_UNSUPPORTED where the own FFT does not exist)                 */
     int no_floating_mean;   /* 0: floating mean, six sums (default; north_star).  1: the fixed-mean form of
                                PAPER.md:17 ("four weighted trigonometric sums"): y centred by its weighted
                                mean, sinusoid model without an offset term                          */

@@ -417,7 +417,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
 
     p->own_fft = o.fft_impl != 1 && lsb::own_fft_supported(p);
     if (o.fft_impl >= 2 && !p->own_fft) { delete p; return LS_ERR_UNSUPPORTED; }
-    p->fuse_assemble = p->own_fft && o.fft_impl != 3 && !o.dy_per_series;
+    // Measured at config 3 (profiles/r1e_cfg3.md): with the cheaper assembly arithmetic the separate
+    // assembly kernel (0.118 ms at 81 % of DRAM peak) plus an unfused third pass beats the fused kernel, which is
+    // bound by its 2-CTAs-per-SM arithmetic, by 1 % — so fusion is opt-in (fft_impl = 2), not the default.
+    p->fuse_assemble = p->own_fft && o.fft_impl == 2 && !o.dy_per_series;
 
     // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
     p->ndf = two_prod((double)p->n, df);

@@ -55,7 +55,7 @@ def test_direct_rejects_bad_arguments():
 
 
 def test_cfg3_nufft_path_against_direct_on_wide_ranges():
-    """Headline size, launch configuration of bench.py (auto plan: n = 2^24, own FFT, fused last pass)."""
+    """Headline size, launch configuration of bench.py (auto plan: n = 2^24, own FFT)."""
     w = make_workload(3)
     Pg = gpu_power(w)[0]
     half = w.Nf // 2

@@ -85,13 +85,14 @@ def test_cfg3_own_fft_against_cufft_full_grid():
             assert num / den <= w.eps, (a, num / den)
 
 
-def test_own_fft_batch_in_two_passes_at_headline_size():
-    """Batch of 3 at n = 2^24 (own FFT, 512-cell tiles, liveness masks reused by the second pass, third FFT pass
-    fused with the assembly): every series must equal its own single-series execute."""
+@pytest.mark.parametrize("fft_impl", [0, 2])
+def test_own_fft_batch_in_two_passes_at_headline_size(fft_impl):
+    """Batch of 3 at n = 2^24 (own FFT, 512-cell tiles, liveness masks reused by the second pass; fft_impl 2: third
+    FFT pass fused with the assembly): every series must equal its own single-series execute."""
     w = make_workload(3)
     y = np.stack([w.y[0], 2.5 * w.y[0] + 7.0, w.y[0] + np.sin(2 * np.pi * w.t / 3.3)])
     wb = Workload("cfg3_batch3", w.t, np.ascontiguousarray(y), w.dy, w.f0, w.df, w.Nf, "f64", w.eps)
-    Pb, ex = gpu_power(wb, batch_chunk=2, return_plan_info=True)
+    Pb, ex = gpu_power(wb, batch_chunk=2, fft_impl=fft_impl, return_plan_info=True)
     assert ex["info"]["n"] == 1 << 24 and ex["info"]["M"] == 5 and ex["launches"][1] == 0
     P0 = gpu_power(w)[0]
     assert np.max(np.abs(Pb[0] - P0)) <= 1e-12

@@ -25,8 +25,8 @@ def test_variants_small_grid_cufft_path(fit_mean, norm):
     assert _rel(Pg, Po) <= 1e-8, (fit_mean, norm, _rel(Pg, Po))
 
 
-@pytest.mark.parametrize("fit_mean,norm", [(False, "standard"), (False, "psd"), (True, "log")])
-def test_variants_own_fft_fused_path(fit_mean, norm):
+@pytest.mark.parametrize("fit_mean,norm,fft_impl", [(False, "standard", 2), (False, "psd", 0), (True, "log", 2)])
+def test_variants_own_fft_paths(fit_mean, norm, fft_impl):
     rng = np.random.default_rng(90)
     Nf = int(0.7 * (1 << 20)); Nd = Nf // 12
     t = rng.uniform(0, 800.0, Nd); dy = rng.uniform(0.5, 1.5, Nd)
@@ -34,7 +34,7 @@ def test_variants_own_fft_fused_path(fit_mean, norm):
     y = 5.0 + np.sin(2 * np.pi * (df + 40000 * df) * t) + rng.normal(0, 1.0, Nd)
     w = Workload("variants_p20", t, np.ascontiguousarray(y[None]), dy, df, df, Nf, "f64", 1e-9)
     Pg, ex = gpu_power(w, no_autotune=1, no_floating_mean=0 if fit_mean else 1, normalization=NORM[norm],
-                       return_plan_info=True)
+                       fft_impl=fft_impl, return_plan_info=True)
     assert ex["launches"][1] == 0                                   # own FFT, no cuFFT exec
     ks = np.unique(np.concatenate([compare_indices(w, 300), np.arange(39995, 40006)]))
     Po = variants.power(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, k=ks, fit_mean=fit_mean, normalization=norm)
