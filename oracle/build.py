@@ -16,6 +16,16 @@ LIB = os.path.join(HERE, "libls_oracle.so")
 
 
 def build(force: bool = False) -> str:
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:          # one builder at a time (torchrun ranks)
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(force: bool) -> str:
     if (not force) and os.path.exists(LIB) and os.path.getmtime(LIB) >= os.path.getmtime(SRC):
         return LIB
     cmd = ["gcc", "-O2", "-std=gnu11", "-fopenmp", "-mfma", "-ffp-contract=off", "-fno-fast-math",

@@ -28,6 +28,18 @@ def _stale(target: str, deps) -> bool:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
+    """Compile what is stale.  Serialised across processes by a file lock: under torchrun every rank calls
+    this, and concurrent nvcc runs must not write the same objects."""
+    import fcntl
+    with open(os.path.join(HERE, ".build.lock"), "w") as lock:
+        fcntl.flock(lock, fcntl.LOCK_EX)
+        try:
+            return _build_locked(force, verbose)
+        finally:
+            fcntl.flock(lock, fcntl.LOCK_UN)
+
+
+def _build_locked(force: bool, verbose: bool) -> str:
     nvcc = os.path.join(CUDA_HOME, "bin", "nvcc")
     objs = []
     for src in SOURCES:
