@@ -94,3 +94,21 @@ def test_cfg5_fp32_path_against_direct_on_ranges():
     rel = np.concatenate(rel)
     assert worst / pmax <= GATE_F32, worst / pmax
     assert np.median(rel) <= 1e-4, np.median(rel)
+
+
+def test_cfg3_julian_date_sized_time_offset_against_direct_and_oracle():
+    """Config 3 with t + 2 450 000.5 (Julian-date-sized times: f t reaches 6e8 cycles, the regime that needs the
+    (cell, fraction) double-double coordinates): NUFFT path vs brute force on two slabs, and both vs the
+    CPU oracle on sampled frequencies of those slabs."""
+    w = make_workload(3)
+    w2 = type(w)(w.name + "_jd", w.t + 2450000.5, w.y, w.dy, w.f0, w.df, w.Nf, "f64", w.eps)
+    Pg = gpu_power(w2)[0]
+    pmax = float(Pg.max())
+    for k0 in (0, w.Nf - (1 << 17)):
+        K = 1 << 17
+        Pd = _direct(w2, k0, K)
+        assert np.max(np.abs(Pg[k0:k0 + K] - Pd)) / pmax <= GATE_F64
+        ks = k0 + np.arange(0, K, 2048)
+        Po = oracle_power(w2, ks=ks)
+        assert np.max(np.abs(Pd[ks - k0] - Po)) / pmax <= 1e-11           # direct vs direct
+        assert np.max(np.abs(Pg[ks] - Po)) / pmax <= GATE_F64
