@@ -352,7 +352,7 @@ ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __rest
 // on the per-series sums stay cheap.
 inline int point_blocks(long long Nd, int batch) {
     const long long want = (Nd + kPreThreads - 1) / kPreThreads;
-    const long long cap = batch >= 64 ? 32 : 148 * 16;
+    const long long cap = std::max<long long>(2, (148 * 16 + batch - 1) / batch);   // ~2400 CTAs over the whole batch
     return (int)(want < cap ? want : cap);
 }
 
