@@ -125,6 +125,25 @@ def test_own_fft_other_power_of_two_grids(p):
     assert int(np.argmax(P_own[0])) == kg
 
 
+def test_own_fft_per_series_dy_and_dense_points():
+    """Own FFT (n = 2^20) with per-series dy (slots [w2_s ...][(w_s, h_s) ...], liveness masks of both point sets) and
+    more points than a spreading chunk holds per tile (several 256-candidate chunks per tile)."""
+    rng = np.random.default_rng(77)
+    Nf = int(0.7 * (1 << 20)); Nd = 400_000                        # ~1.9 points per cell in the occupied fifth
+    t = rng.uniform(0, 1000.0, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    y = np.stack([np.sin(2 * np.pi * (df + 50_000 * df) * t) + rng.normal(0, 1, Nd),
+                  0.5 * np.cos(2 * np.pi * (df + 300_000 * df) * t) + rng.normal(0, 1, Nd)])
+    dy = rng.uniform(0.5, 1.5, (2, Nd))
+    w = Workload("own_fft_per_series", t, np.ascontiguousarray(y), np.ascontiguousarray(dy), df, df, Nf, "f64", 1e-9)
+    Pg, ex = gpu_power(w, no_autotune=1, return_plan_info=True)
+    assert ex["info"]["n"] == 1 << 20 and ex["info"]["M"] == 6 and ex["launches"][1] == 0
+    for b, kg in ((0, 50_000), (1, 300_000)):
+        ks = np.unique(np.concatenate([compare_indices(w, 150), np.arange(kg - 3, kg + 4)]))
+        _check64(errors(Pg[b][ks], oracle_power(w, b, ks=ks)))
+        assert int(np.argmax(Pg[b])) == kg
+
+
 def test_own_fft_rejected_where_unsupported():
     from gpu_util import require_cuda
     require_cuda()
