@@ -18,8 +18,8 @@
  *
  * Every step runs in hand-written sm_100a kernels (stats, bin-count + scan, premultiply-scatter,
  * tile-owner spread, deconvolve + assemble).  The fine-grid FFT is the library's own three-pass
- * transform for fp64 grids of 2^20..2^24 cells (pruned first pass, last pass fused with the
- * assembly) and one cuFFT plan for every other grid.  There is NO CPU fallback: every entry point
+ * transform for fp64 power-of-two grids of 2^12..2^24 cells (first pass pruned from 2^20 cells on)
+ * and one cuFFT plan for every other grid.  There is NO CPU fallback: every entry point
  * fails with LS_ERR_CUDA when no device is usable.
  *
  * Conventions
@@ -92,8 +92,8 @@ typedef struct {
     int graph;              /* CUDA-graph replay of the execute sequence (needs timing == 0 and a non-legacy
                                stream): 0 = auto (on; off for good after three consecutive executes
                                with changed buffer pointers), 1 = never, 2 = always                 */
-    int fft_impl;           /* 0 = auto (the library's own three-pass FFT where it exists — fp64 grids of
-                               2^20..2^24 cells — else cuFFT), 1 = cuFFT plan, 2 = own FFT with the h
+    int fft_impl;           /* 0 = auto (the library's own three-pass FFT where it exists — fp64 power-of-two grids
+                               of 2^12..2^24 cells; in auto mode not for large batches of small grids — else cuFFT), 1 = cuFFT plan, 2 = own FFT with the h
                                transforms' last pass fused with deconvolution + assembly, 3 = own FFT
                                with the assembly as a separate kernel (what auto picks; 2 and 3 give
                                LS_ERR_UNSUPPORTED where the own FFT does not exist)                 */

@@ -415,7 +415,12 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     }
     p->slots = per ? 3 * p->chunk : 2 + p->chunk;
 
+    // own FFT: wherever it exists when asked for (fft_impl 2, 3); in auto mode for the pruned sizes (n >= 2^20) and, below
+    // them, for problems small enough to be latency-bound (cuFFT runs a 2^14-point fp64 transform in ONE CTA: 29 us of
+    // config 1's 58), but not for large batches of small grids, where cuFFT's pass structure moves fewer bytes
     p->own_fft = o.fft_impl != 1 && lsb::own_fft_supported(p);
+    if (p->own_fft && o.fft_impl == 0 && !lsb::own_fft_prunes(p) && (double)p->M * (double)p->n * 16.0 > 64e6) p->own_fft = false;
+    p->fft_prune = p->own_fft && lsb::own_fft_prunes(p);
     if (o.fft_impl >= 2 && !p->own_fft) { delete p; return LS_ERR_UNSUPPORTED; }
     // Measured at config 3 (profiles/r1e_cfg3.md): with the cheaper assembly arithmetic the separate
     // assembly kernel (0.118 ms at 81 % of DRAM peak) plus an unfused third pass beats the fused kernel, which is
@@ -447,10 +452,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
-        const size_t mask_bytes = p->own_fft ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : 0;   // masks + 2 list counters
+        const size_t mask_bytes = p->fft_prune ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : 0;   // masks + 2 list counters
         p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
-        if (p->own_fft) {
+        if (p->fft_prune) {
             p->tile_counts = (int*)((char*)p->zeroed + sums_bytes + hist_bytes);
             p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes + 256);
             if ((ce = dmalloc(p, &p->tile_list, (size_t)2 * p->ntiles * 4)) != cudaSuccess) break;
@@ -548,7 +553,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
 
     stage_begin(p, LS_STAGE_SORT, s);
     LS_TRY(lsb::launch_bin_scan(p, s)); own += 2;
-    if (p->own_fft) { LS_TRY(lsb::launch_tile_list(p, s)); ++own; }
+    if (p->fft_prune) { LS_TRY(lsb::launch_tile_list(p, s)); ++own; }
     stage_end(p, s);
 
     stage_begin(p, LS_STAGE_PREMUL, s);
@@ -589,7 +594,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 stage_begin(p, LS_STAGE_FFT_PASS3, s);
                 LS_TRY(lsb::launch_own_fft_pass3(p, ps.fft_slot0, n_modes, s));
                 stage_end(p, s);
-                own += n_modes > 0 ? 3 : 2;
+                own += 1 + (p->n > 65536 ? 1 : 0) + (n_modes > 0 ? 1 : 0);
             } else {
                 stage_begin(p, LS_STAGE_FFT, s);
                 cufftHandle h = find_fft(p, ps.fft_batch);

@@ -1,10 +1,10 @@
-// ls_fft.cu — the library's own fine-grid FFT for complex128 grids of n = 2^20 .. 2^24 cells (
+// ls_fft.cu — the library's own fine-grid FFT for complex128 grids of n = 2^12 .. 2^24 cells (
 // PAPER.md:47 "use an equispaced FFT", :73 "the FFT time dominates").
 //
 //   B_k = sum_l b_l e^{+2 pi i k l / n}     (reading A7: the unnormalised inverse transform)
 //
-// Three passes over n = R1 R2 R3, R2 = R3 = 256, R1 = n / 2^16 = 16 .. 256 (256^3 at the headline size),
-// decimation in frequency:
+// Three passes over n = R1 R2 R3, R2 = R3 = 256, R1 = n / 2^16 = 2 .. 256 (256^3 at the headline size; two passes
+// R1 x 256 for n <= 2^16), decimation in frequency:
 //   l = l1 R2 R3 + l2 R3 + l3,   k = k1 + R1 k2 + R1 R2 k3
 //   pass 1: FFT over l1 -> k1, times w_n^{k1 (l2 R3 + l3)};   in place, layout [k1][l2][l3]
 //   pass 2: FFT over l2 -> k2, times w_n^{R1 k2 l3};          in place, layout [k1][k2][l3]
@@ -103,7 +103,8 @@ __device__ __forceinline__ void fft_small(double2 (&x)[RB]) {
 struct FftArgs {
     double2* grids;            // [ntrans][n] in place
     long long n;
-    int R1, R2, R3;            // n = R1 * 256 * 256, R1 = 16 RB in {16 .. 256}
+    int R1, R2, R3;            // n = R1 R2 R3; R3 = 256; R2 = 256 (three passes) or 1 (two passes); R1 a power of two
+    int R1_shift;              // log2(R1)
     const double2* wlo;        // w_n^x, x < 4096
     const double2* whi;        // w_n^{4096 y}, y < n / 4096
     // pass 1 pruning (see PointSet-independent `row_masks` in ls_internal.h): for point set s, spreading-tile
@@ -200,6 +201,7 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
     const int c = threadIdx.x % C, hi = threadIdx.x / C;     // hi: j in stage 1, item group in stage 2
     auto mask_of = [&](int tile) -> unsigned {
         if (tile >= ntiles_total) return 0u;
+        if (a.row_masks == nullptr) return 0xffffu;          // unpruned: every row was written
         const int tr = tile / tiles_per_trans;
         const long long m0 = (long long)(tile - tr * tiles_per_trans) * C;
         const int set = tr < a.set_of_trans_first ? 0 : 1;
@@ -252,6 +254,27 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
     }
 }
 
+// First pass for n = 2^17 .. 2^19 (R1 = 2, 4, 8 rows of 65536 cells): one thread per column, R1-point FFT in
+// registers, times w_n^{k1 m}; in place.  Memory-bound by construction.
+template <int R>
+__global__ void __launch_bounds__(256)
+ls_fft_pass1_small_kernel(const FftArgs a, long long inner) {
+    const int tr = blockIdx.y;
+    double2* base = a.grids + (long long)tr * a.n;
+    for (long long m = (long long)blockIdx.x * blockDim.x + threadIdx.x; m < inner; m += (long long)gridDim.x * blockDim.x) {
+        double2 x[R];
+#pragma unroll
+        for (int i = 0; i < R; ++i) x[i] = base[(long long)i * inner + m];
+        fft_small<R>(x);
+#pragma unroll
+        for (int k1 = 0; k1 < R; ++k1) {
+            double2 v = x[fft_pos<R>(k1)];
+            if (k1 > 0) v = cmul(v, twiddle_n(a, (unsigned)k1 * (unsigned)m));
+            base[(long long)k1 * inner + m] = v;
+        }
+    }
+}
+
 // Pass 3: the transform dimension (l3) is contiguous; the CTA takes 16 consecutive k1 at one k2, so that the
 // kept modes leave in runs of 16 consecutive frequencies.  Output: modes[tr][k], k = (kk + half) mod n < Nf,
 // kk = k1 + R1 k2 + R1 R2 k3 the stored mode index (= k' mod n).
@@ -264,12 +287,14 @@ ls_fft_rows_kernel(const FftArgs a) {
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][17] (padded: conflict-free both ways)
     double2* w256 = Y + 256 * (kC + 1);
     fill_w256(w256);
-    const int k1b = blockIdx.x * kC, k2 = blockIdx.y, tr = blockIdx.z;
+    // rows are numbered rho = k1 + R1 k2 (the low part of the output index): 16 consecutive rho per CTA
+    const int rho_b = blockIdx.x * kC, tr = blockIdx.z;
     const double2* src = a.grids + (long long)tr * a.n;
     double2 x[16];
     {
         const int j = threadIdx.x & 15, c = threadIdx.x >> 4;
-        const double2* row = src + ((long long)(k1b + c) * a.R2 + k2) * a.R3;
+        const int rho = rho_b + c, k1 = rho & (a.R1 - 1), k2 = rho >> a.R1_shift;
+        const double2* row = src + ((long long)k1 * a.R2 + k2) * a.R3;
 #pragma unroll
         for (int i = 0; i < 16; ++i) x[i] = row[16 * i + j];
         fft16(x);
@@ -284,7 +309,7 @@ ls_fft_rows_kernel(const FftArgs a) {
         for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * (kC + 1) + c];
         fft16(x);
         double2* out = a.modes + (long long)tr * a.Nf;
-        const long long kk0 = (long long)(k1b + c) + (long long)a.R1 * k2;
+        const long long kk0 = rho_b + c;
         const long long r12 = (long long)a.R1 * a.R2;
         const int ser = a.series0 + tr;
         const double YYs = FUSED ? a.sums[4 * ser + 2] : 1.0;
@@ -352,13 +377,19 @@ constexpr size_t kRowsSmem = sizeof(double2) * (256 * (kC + 1) + 256);
 
 }  // namespace
 
-// fp64 grids of 2^20 .. 2^24 cells: n = R1 * 256 * 256 with R1 = 16 .. 256 (pass 1 radix), spreading tiles that
-// divide a pass-1 row of 65536 cells.
+// fp64 grids of n = 2^12 .. 2^24 cells:
+//   2^20 .. 2^24: three passes R1 x 256 x 256, R1 = 16 .. 256, first pass pruned by the spreading kernel's liveness
+//                 masks (needs spreading tiles that divide a pass-1 row of 65536 cells);
+//   2^17 .. 2^19: three passes with a small first radix R1 = 2, 4, 8 (ls_fft_pass1_small_kernel), unpruned;
+//   2^12 .. 2^16: two passes R1 x 256, R1 = 16 .. 256, unpruned.
 bool own_fft_supported(const ls_plan_s* p) {
     const bool pow2 = (p->n & (p->n - 1)) == 0;
-    return p->dtype == LS_F64 && pow2 && p->n >= ((int64_t)1 << 20) && p->n <= ((int64_t)1 << 24) && 65536 % p->L == 0;
+    if (p->dtype != LS_F64 || !pow2 || p->n < ((int64_t)1 << 12) || p->n > ((int64_t)1 << 24)) return false;
+    return p->n < ((int64_t)1 << 20) || 65536 % p->L == 0;
 }
-int own_fft_rb(const ls_plan_s* p) { return (int)(p->n >> 20); }
+bool own_fft_prunes(const ls_plan_s* p) { return p->n >= ((int64_t)1 << 20); }
+// radix of the first pass / 16 where that pass is the 16 x RB kernel (n >= 2^20: R1 = n / 2^16; n <= 2^16: R1 = n / 2^8)
+int own_fft_rb(const ls_plan_s* p) { return (int)(p->n >= ((int64_t)1 << 20) ? p->n >> 20 : p->n >> 12); }
 
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     const int cnt = (int)std::max<long long>(4096, p->n / 4096);
@@ -379,12 +410,15 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
 static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.grids = (double2*)p->grids + (long long)slot0 * p->n;
     a.n = p->n;
-    a.R1 = (int)(p->n >> 16);
-    a.R2 = a.R3 = 256;
+    a.R3 = 256;
+    a.R2 = p->n > 65536 ? 256 : 1;                         // two passes up to 2^16 cells
+    a.R1 = (int)(p->n / ((long long)a.R2 * a.R3));
+    a.R1_shift = 0;
+    while ((1 << a.R1_shift) < a.R1) ++a.R1_shift;
     a.wlo = (const double2*)p->fft_wlo;
     a.whi = (const double2*)p->fft_whi;
-    a.row_masks = p->row_masks;
-    a.ncoltiles = 65536 / p->L;
+    a.row_masks = own_fft_prunes(p) ? p->row_masks : nullptr;
+    a.ncoltiles = std::max(1, 65536 / p->L);
     a.set_of_trans_first = n_x2;
     a.tile_shift = 0;
     while ((1 << a.tile_shift) < p->L) ++a.tile_shift;
@@ -405,7 +439,14 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot0, n_x2);
-    const long long inner1 = 65536;
+    const long long inner1 = (long long)a.R2 * a.R3;       // 65536 (three passes) or 256 (two passes)
+    if (a.R1 < 16) {                                       // n = 2^17 .. 2^19
+        dim3 g((unsigned)std::min<long long>((inner1 + 255) / 256, 4LL * p->num_sms), ntrans);
+        if (a.R1 == 8) ls_fft_pass1_small_kernel<8><<<g, 256, 0, s>>>(a, inner1);
+        else if (a.R1 == 4) ls_fft_pass1_small_kernel<4><<<g, 256, 0, s>>>(a, inner1);
+        else ls_fft_pass1_small_kernel<2><<<g, 256, 0, s>>>(a, inner1);
+        return cudaGetLastError();
+    }
     const int rb = own_fft_rb(p);
     const int tiles_per_trans = (int)(inner1 / (256 / rb)), total = tiles_per_trans * ntrans;
     const int nblk = std::min(total, (512 / kFftThreads) * p->num_sms);
@@ -422,6 +463,7 @@ cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, 
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot0, 0);
+    if (a.R2 == 1) return cudaSuccess;                     // two-pass sizes: nothing between pass 1 and the last pass
     dim3 g2(256 / kC, a.R1, ntrans);                       // [k1][l2][l3]: outer = R1 blocks, stride 256
     ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, a.R1, 256);
     return cudaGetLastError();
@@ -432,7 +474,7 @@ cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream
     if (ntrans <= 0) return cudaSuccess;
     FftArgs a;
     fill_common(p, a, slot0, 0);
-    dim3 g3(a.R1 / kC, 256, ntrans);
+    dim3 g3(a.R1 * a.R2 / kC, 1, ntrans);
     ls_fft_rows_kernel<false><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
 }
@@ -447,7 +489,7 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
     a.w2_modes = (const double2*)p->modes + (long long)w2_slot * p->Nf;
     a.power = (double*)power;
     a.series0 = series0;
-    dim3 g3(a.R1 / kC, 256, nseries);
+    dim3 g3(a.R1 * a.R2 / kC, 1, nseries);
     if (a.no_float || a.norm) ls_fft_rows_kernel<true, true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     else ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();

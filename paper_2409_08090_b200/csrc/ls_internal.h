@@ -110,6 +110,7 @@ struct ls_plan_s {
     bool external_ws = false;   // grids / modes / fft_work live in caller memory (ls_set_workspace)
     // own FFT (ls_fft.cu): n = 2^20 .. 2^24, fp64; opts.fft_impl
     bool own_fft = false;
+    bool fft_prune = false;                         // spreading skips empty tiles, FFT pass 1 prunes by liveness masks
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
     void* modes = nullptr;                          // [slots][Nf] complex: kept modes in frequency order
@@ -146,7 +147,8 @@ int spread_rows_per_group(const ls_plan_s* p);
 cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s);
 // ---- ls_fft.cu: own three-pass FFT (n = 2^20 .. 2^24, fp64) ------------------------------------------
 bool own_fft_supported(const ls_plan_s* p);
-int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 = n / 2^20
+bool own_fft_prunes(const ls_plan_s* p);          // first pass pruned by liveness masks (n >= 2^20)
+int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 (where that pass is the 16 x RB kernel)
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s);
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);

@@ -478,13 +478,13 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.tile_stride = p->tile_stride;
     a.tile_mask = (p->ntiles & (p->ntiles - 1)) == 0 ? p->ntiles - 1 : -1;
     a.half = p->poly.half;
-    a.skip_empty = p->own_fft ? 1 : 0;
+    a.skip_empty = p->fft_prune ? 1 : 0;
     a.row_masks = p->row_masks;
     a.tile_list = p->tile_list;
     a.w_implicit = p->opts.dy_per_series ? 0 : 1;
     a.tile_counts = p->tile_counts;
     a.ncoltiles = std::max(1, 65536 / p->L);
-    a.fft_rb = p->own_fft ? own_fft_rb(p) : 1;
+    a.fft_rb = p->fft_prune ? own_fft_rb(p) : 1;
     a.coltile_shift = 0;
     while ((1 << a.coltile_shift) < a.ncoltiles) ++a.coltile_shift;
     a.Nd = p->Nd;

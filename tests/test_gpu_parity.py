@@ -37,7 +37,7 @@ def test_cfg1_full_grid():
     e = errors(Pg[0], Po)
     _check64(e)
     assert int(np.argmax(Pg[0])) == int(np.argmax(Po))
-    assert ex["launches"][0] > 0 and ex["launches"][1] == 1            # our kernels ran; one cuFFT exec
+    assert ex["launches"][0] > 0 and ex["launches"][1] == 0            # our kernels ran, own FFT included (n = 2^14)
     assert ex["info"]["M"] == 3 and ex["info"]["n"] >= 1.25 * w.Nf
 
 
@@ -103,13 +103,13 @@ def test_own_fft_batch_in_two_passes_at_headline_size(fft_impl):
     _check64(errors(Pb[2][ks], oracle_power(w2, ks=ks)))
 
 
-@pytest.mark.parametrize("p", [20, 21, 22, 23])
+@pytest.mark.parametrize("p", [12, 13, 14, 15, 16, 17, 18, 19, 20, 21, 22, 23])
 def test_own_fft_other_power_of_two_grids(p):
-    """n = 2^p, p = 20..23: first-pass radix 16, 32, 64, 128 (ls_fft_pass1_kernel<RB>), against cuFFT on the
-    full grid and against the oracle on sampled frequencies."""
+    """n = 2^p: two passes R1 x 256 (p = 12..16), three passes with a first radix of 2, 4, 8 (p = 17..19) or of
+    16..128 with pruning (p = 20..23), against cuFFT on the full grid and against the oracle on sampled k."""
     rng = np.random.default_rng(400 + p)
     Nf = int(0.7 * (1 << p))
-    Nd = Nf // 12
+    Nd = max(200, Nf // 12)
     t = rng.uniform(0, 2000.0, Nd)
     dy = rng.uniform(0.5, 1.5, Nd)
     df = 1.0 / (5 * (t.max() - t.min()))
@@ -149,7 +149,13 @@ def test_own_fft_rejected_where_unsupported():
     require_cuda()
     from paper_2409_08090_b200 import binding as B
     with pytest.raises(B.LsError) as ei:
-        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=2)     # n = 2^14
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-5, B.LS_F32, 1, fft_impl=2)     # fp32 grid
+    assert ei.value.code == 5
+    with pytest.raises(B.LsError) as ei:
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=2, upsampfac=1.5)   # n = 18750, not a power of two
+    assert ei.value.code == 5
+    with pytest.raises(B.LsError) as ei:
+        B.Plan(100, 1000, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=3)       # n = 2048 < 2^12
     assert ei.value.code == 5
     with pytest.raises(B.LsError) as ei:
         B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, fft_impl=4)
