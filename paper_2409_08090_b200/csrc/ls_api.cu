@@ -552,7 +552,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
     stage_end(p, s);
 
     stage_begin(p, LS_STAGE_SORT, s);
-    LS_TRY(lsb::launch_bin_scan(p, s)); own += 2;
+    LS_TRY(lsb::launch_bin_scan(p, s)); own += p->nbins > 4096 ? 2 : 1;
     if (p->fft_prune) { LS_TRY(lsb::launch_tile_list(p, s)); ++own; }
     stage_end(p, s);
 

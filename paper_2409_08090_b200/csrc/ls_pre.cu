@@ -219,6 +219,30 @@ ls_bin_scan_apply_kernel(int* __restrict__ hist1, int* __restrict__ hist2, int* 
     if (blockIdx.x == 0 && threadIdx.x == 0) start[nbins] = Nd;
 }
 
+// Small grids (all bins of a point set fit one chunk): both phases in one launch.
+__global__ void __launch_bounds__(kScanThreads)
+ls_bin_scan_single_kernel(int* __restrict__ hist1, int* __restrict__ hist2, int* __restrict__ start1,
+                          int* __restrict__ start2, int nbins, int Nd) {
+    __shared__ int warp_tot[33];
+    int* hist = blockIdx.y ? hist2 : hist1;
+    int* start = blockIdx.y ? start2 : start1;
+    const int b0 = threadIdx.x * kScanItems;
+    int v[kScanItems];
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) v[i] = (b0 + i < nbins) ? hist[b0 + i] : 0;
+    int total;
+    int ex = chunk_exclusive_scan(v, warp_tot, total);
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        if (b0 + i < nbins) {
+            start[b0 + i] = ex;
+            hist[b0 + i] = ex;                   // the counts become the scatter cursors
+        }
+        ex += v[i];
+    }
+    if (threadIdx.x == 0) start[nbins] = Nd;
+}
+
 // ------------------------------------------------------------------------------ K2 premultiply
 template <typename T>
 struct RecOf;
@@ -374,6 +398,11 @@ cudaError_t launch_stats_count(ls_plan_s* p, const double* t, const void* y, con
 cudaError_t launch_bin_scan(ls_plan_s* p, cudaStream_t s) {
     const int nchunks = (p->nbins + kScanChunk - 1) / kScanChunk;
     dim3 grid(nchunks, 2);
+    if (nchunks == 1) {
+        ls_bin_scan_single_kernel<<<grid, kScanThreads, 0, s>>>(p->ps[0].hist, p->ps[1].hist, p->ps[0].bin_start,
+                                                               p->ps[1].bin_start, p->nbins, (int)p->Nd);
+        return cudaGetLastError();
+    }
     ls_bin_scan_totals_kernel<<<grid, kScanThreads, 0, s>>>(p->ps[0].hist, p->ps[1].hist, p->nbins, nchunks,
                                                             p->scan_tmp);
     cudaError_t e = cudaGetLastError();
