@@ -251,9 +251,9 @@ def stage_model_bytes(w, info, own_fft, L):
 
 def measured_traffic(kernel_stage, w, info):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    ncu --set full capture (profiles/r1e_traffic.csv; same command line, config 3 defaults).  None when
+    ncu --set full capture (profiles/r1f_traffic.csv; same command line, config 3 defaults).  None when
     the capture does not cover this workload / plan."""
-    path = os.path.join(ROOT, "profiles", "r1e_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r1f_traffic.csv")
     try:
         with open(path) as f:
             rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
