@@ -101,7 +101,9 @@ typedef struct {
                                PAPER.md:17 ("four weighted trigonometric sums"): y centred by its weighted
                                mean, sinusoid model without an offset term                          */
     int normalization;      /* LS_NORM_STANDARD (default), _MODEL, _LOG, _PSD            */
-    int reserved[3];        /* must be zero                                                       */
+    int t_is_dtype;         /* 0: t is double[Nd] (default, recommended: A9).  1 with LS_F32: t is float[Nd]; it is
+                               promoted exactly to double on the device before anything else reads it  */
+    int reserved[2];        /* must be zero                                                       */
 } ls_opts;
 
 /* ls_plan — choose (sigma, w, beta, n) from eps ("width and fine grid size are
@@ -115,7 +117,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
             int dtype, int batch, const ls_opts* opts /* NULL ok */);
 
 /* ls_execute — one pass of the whole hot path (§8(a) K1..K6 + cuFFT) for `batch` series.
- *   t      device, const double[Nd]
+ *   t      device, const double[Nd]  (const float[Nd] with opts.t_is_dtype on an LS_F32 plan)
  *   y      device, const dtype[batch][Nd]
  *   dy     device, const dtype[Nd] (or [batch][Nd] with opts.dy_per_series)
  *   power  device, dtype[batch][Nf]   (written)

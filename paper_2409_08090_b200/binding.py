@@ -41,7 +41,8 @@ class ls_opts(C.Structure):
         ("fft_impl", C.c_int),
         ("no_floating_mean", C.c_int),
         ("normalization", C.c_int),
-        ("reserved", C.c_int * 3),
+        ("t_is_dtype", C.c_int),
+        ("reserved", C.c_int * 2),
     ]
 
 

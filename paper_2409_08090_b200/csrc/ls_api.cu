@@ -299,6 +299,7 @@ int ls_destroy(ls_plan_t p) {
         cudaFree(p->modes);
     }
     cudaFree(p->dinv);
+    cudaFree(p->t64);
     cudaFree(p->fft_wlo);
     cudaFree(p->fft_whi);
     cudaFree(p->tile_list);
@@ -340,6 +341,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
                               o.tile_cells > lsb::kSpreadThreads * 4))
         return LS_ERR_INVALID_VALUE;
+    if (o.t_is_dtype < 0 || o.t_is_dtype > 1) return LS_ERR_INVALID_VALUE;
     if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 3 ||
         o.no_floating_mean < 0 || o.no_floating_mean > 1 || o.normalization < 0 || o.normalization > 3)
         return LS_ERR_INVALID_VALUE;
@@ -442,6 +444,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         p->grids_bytes = (size_t)p->slots * grid_bytes;
         if ((ce = dmalloc(p, &p->grids, p->grids_bytes)) != cudaSuccess) break;
         if ((ce = dmalloc(p, &p->dinv, (size_t)(Nf / 2 + 1) * 8)) != cudaSuccess) break;
+        if (o.t_is_dtype && dtype == LS_F32 && (ce = dmalloc(p, &p->t64, (size_t)Nd * 8)) != cudaSuccess) break;
         if (p->own_fft) {
             if ((ce = dmalloc(p, (char**)&p->fft_wlo, (size_t)4096 * 16)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&p->fft_whi, (size_t)std::max<int64_t>(4096, p->n / 4096) * 16)) != cudaSuccess) break;
@@ -547,6 +550,10 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
     if (p->opts.timing) ++p->events_used;
 
     stage_begin(p, LS_STAGE_STATS, s);              // K1 + the bin histogram of K3 (one kernel)
+    if (p->t64) {                                   // float times: promoted once, read as double from here on
+        LS_TRY(lsb::launch_promote_t(p, t, s)); ++own;
+        t = p->t64;
+    }
     LS_TRY(cudaMemsetAsync(p->zeroed, 0, p->zeroed_bytes, s));
     LS_TRY(lsb::launch_stats_count(p, (const double*)t, y, dy, s)); ++own;
     stage_end(p, s);
@@ -668,7 +675,7 @@ int ls_execute_host(ls_plan_t p, const void* t, const void* y, const void* dy, v
     if (!p || !t || !y || !dy || !power) return LS_ERR_INVALID_VALUE;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     const size_t B = real_bytes(p->dtype);
-    const size_t bt = (size_t)p->Nd * 8, by = (size_t)p->batch * p->Nd * B;
+    const size_t bt = (size_t)p->Nd * (p->t64 ? 4 : 8), by = (size_t)p->batch * p->Nd * B;
     const size_t bdy = (size_t)(p->opts.dy_per_series ? p->batch : 1) * p->Nd * B;
     const size_t bp = (size_t)p->batch * p->Nf * B;
     if (!p->st_t) {

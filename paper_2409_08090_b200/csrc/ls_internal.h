@@ -91,6 +91,7 @@ struct ls_plan_s {
     // device buffers
     void* grids = nullptr;      // [slots][n] complex T
     double* dinv = nullptr;     // [floor(Nf/2)+1] 1/psihat(k')
+    double* t64 = nullptr;      // [Nd] times promoted from float (opts.t_is_dtype on an LS_F32 plan)
     double* sums = nullptr;     // [batch][4]  (sum dy^-2, sum dy^-2 y, YY, unused); first part of `zeroed`
     void* zeroed = nullptr;     // sums + both histograms: one allocation, one memset per execute
     size_t zeroed_bytes = 0;
@@ -134,6 +135,7 @@ struct ls_plan_s {
 namespace lsb {
 
 // ---- ls_pre.cu: K1 stats + K3 bin count, K3 scan, K2 premultiply + scatter (+ rows) -------
+cudaError_t launch_promote_t(ls_plan_s* p, const void* t_f32, cudaStream_t s);
 cudaError_t launch_stats_count(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s);
 cudaError_t launch_bin_scan(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_premultiply(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s);

@@ -73,6 +73,12 @@ __device__ __forceinline__ void support_start(double frac, int w, int& i0, doubl
     x0 = a - frac;
 }
 
+// opts.t_is_dtype: float times promoted exactly to double once, so every kernel below reads double times
+__global__ void ls_promote_t_kernel(const float* __restrict__ tf, double* __restrict__ td, long long Nd) {
+    for (long long j = (long long)blockIdx.x * blockDim.x + threadIdx.x; j < Nd; j += (long long)gridDim.x * blockDim.x)
+        td[j] = (double)tf[j];
+}
+
 // ------------------------------------------------------------------------------ K1 stats + K3 count
 // grid (point CTAs, batch), grid-stride over the points.  Every series accumulates sum dy^-2 y (and
 // sum dy^-2 when it has its own dy); the CTAs of series 0 also histogram the fine-grid bins of both
@@ -381,6 +387,11 @@ inline int point_blocks(long long Nd, int batch) {
 }
 
 }  // namespace
+
+cudaError_t launch_promote_t(ls_plan_s* p, const void* t_f32, cudaStream_t s) {
+    ls_promote_t_kernel<<<point_blocks(p->Nd, 1), kPreThreads, 0, s>>>((const float*)t_f32, p->t64, p->Nd);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_stats_count(ls_plan_s* p, const double* t, const void* y, const void* dy, cudaStream_t s) {
     dim3 grid(point_blocks(p->Nd, p->batch), p->batch);

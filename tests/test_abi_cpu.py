@@ -48,7 +48,8 @@ def test_ls_opts_layout_matches_header():
     assert ls_opts.fft_impl.offset == 44
     assert ls_opts.no_floating_mean.offset == 48
     assert ls_opts.normalization.offset == 52
-    assert ls_opts.reserved.offset == 56
+    assert ls_opts.t_is_dtype.offset == 56
+    assert ls_opts.reserved.offset == 60
     assert ctypes.sizeof(ls_opts) == 72
 
 

@@ -464,3 +464,24 @@ def test_invalid_arguments_are_rejected():
     assert ei.value.code == 6
     B.ls_destroy(h)
     B.ls_destroy(None)                                                 # NULL accepted
+
+
+def test_times_given_in_float32():
+    """opts.t_is_dtype on an fp32 plan: t is float[Nd], promoted exactly on the device; the oracle gets the same
+    rounded times."""
+    import torch
+    from paper_2409_08090_b200 import binding as B
+    w = scaled_workload(5, 20_000)
+    tf = w.t.astype(np.float32)
+    w32 = Workload(w.name + "_t32", tf.astype(np.float64), w.y, w.dy, w.f0, w.df, w.Nf, "f32", w.eps)
+    dev = torch.device("cuda:0")
+    P = torch.empty((1, w.Nf), dtype=torch.float32, device=dev)
+    with B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F32, 1, t_is_dtype=1) as plan:
+        plan.execute(torch.from_numpy(tf).to(dev), torch.from_numpy(w.y).to(dev), torch.from_numpy(w.dy).to(dev), P,
+                     torch.cuda.current_stream().cuda_stream)
+        torch.cuda.synchronize()
+    Pg = P.cpu().numpy()[0].astype(np.float64)
+    assert np.max(np.abs(Pg - gpu_power(w32)[0])) <= 1e-6             # same as handing the promoted doubles
+    ks = compare_indices(w32, 1024)
+    e = errors(Pg[ks], oracle_power(w32, ks=ks))
+    assert e["Einf"] <= GATE_F32, e
