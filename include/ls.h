@@ -26,12 +26,16 @@
  *   - All functions return an int status (LS_OK == 0); nothing throws, prints or exits.
  *   - Pointers passed to ls_execute are DEVICE pointers; to ls_execute_host they are HOST
  *     pointers.  The caller owns them; the library never frees or writes inputs.
- *   - Layouts (row-major, contiguous):  t[Nd] (always double);  y[batch][Nd], power[batch][Nf]
- *     in `dtype`;  dy[Nd] (shared by the batch) or dy[batch][Nd] when opts.dy_per_series.
+ *   - Layouts (row-major, contiguous):  t[Nd] (double; float only with opts.t_is_dtype on an
+ *     LS_F32 plan);  y[batch][Nd], power[batch][Nf] in `dtype`;  dy[Nd] (shared by the batch) or
+ *     dy[batch][Nd] when opts.dy_per_series.
  *     power[b][k] is the periodogram of series b at f0 + k*df.
  *   - ls_execute only ENQUEUES work on `cuda_stream` (a cudaStream_t; NULL = legacy default
  *     stream) and returns; it performs no device synchronisation.  One execute may be in flight
  *     per plan (plan-owned scratch); use one plan per stream for concurrency.
+ *   - ls_plan makes opts.device the calling thread's current device and leaves it so; ls_execute,
+ *     ls_execute_host and ls_direct_power expect the plan's device to be current and `cuda_stream`
+ *     to belong to it (they never switch devices themselves).
  *   - dy_j <= 0 or non-finite inputs give undefined (NaN-propagating) output; there is no
  *     device-side validation on the hot path.
  */

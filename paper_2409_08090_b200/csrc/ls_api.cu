@@ -678,9 +678,11 @@ int ls_execute_host(ls_plan_t p, const void* t, const void* y, const void* dy, v
     const size_t bt = (size_t)p->Nd * (p->t64 ? 4 : 8), by = (size_t)p->batch * p->Nd * B;
     const size_t bdy = (size_t)(p->opts.dy_per_series ? p->batch : 1) * p->Nd * B;
     const size_t bp = (size_t)p->batch * p->Nf * B;
-    if (!p->st_t) {
-        if (dmalloc(p, (char**)&p->st_t, bt) != cudaSuccess || dmalloc(p, (char**)&p->st_y, by) != cudaSuccess ||
-            dmalloc(p, (char**)&p->st_dy, bdy) != cudaSuccess || dmalloc(p, (char**)&p->st_p, bp) != cudaSuccess) {
+    if (!p->st_p) {                                   // staging buffers, made on first use; st_p is the last one made
+        if ((!p->st_t && dmalloc(p, (char**)&p->st_t, bt) != cudaSuccess) ||
+            (!p->st_y && dmalloc(p, (char**)&p->st_y, by) != cudaSuccess) ||
+            (!p->st_dy && dmalloc(p, (char**)&p->st_dy, bdy) != cudaSuccess) ||
+            dmalloc(p, (char**)&p->st_p, bp) != cudaSuccess) {
             cudaGetLastError();
             return LS_ERR_ALLOC;
         }
