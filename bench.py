@@ -245,15 +245,17 @@ def stage_model_bytes(w, info, own_fft, L):
         "assemble": M * Nf * 2 * B + batch * Nf * B + (Nf // 2 + 1) * 8,
     }
     if own_fft:
-        d.update({"fft_pass1": written + grid, "fft_pass2": 2 * grid, "fft_pass3": grid + M * Nf * 2 * B})
+        d.update({"fft_pass1": written + grid, "fft_pass2": 2 * grid, "fft_pass3": grid + M * Nf * 2 * B,
+                  # passes 2 + 3 as one kernel, intermediate in L2 and discarded: grid in, kept modes out
+                  "fft_pass23": grid + M * Nf * 2 * B})
     return d
 
 
 def measured_traffic(kernel_stage, w, info):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    ncu --set full capture (profiles/r1f_traffic.csv; same command line, config 3 defaults).  None when
+    ncu --set full capture (profiles/r1g_traffic.csv; same command line, config 3 defaults).  None when
     the capture does not cover this workload / plan."""
-    path = os.path.join(ROOT, "profiles", "r1f_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r1g_traffic.csv")
     try:
         with open(path) as f:
             rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
@@ -382,7 +384,12 @@ def run_ours(args):
     own_fft = ffts == 0
     L = args.tile_cells or (1024 if w.batch == 1 else 512)
     sbytes = stage_model_bytes(w, info, own_fft, L)
-    own_stages = ["stats", "sort", "premul", "spread", "assemble"] + (["fft_pass1", "fft_pass2", "fft_pass3"] if own_fft else [])
+    fused23 = own_fft and info["n"] >= 1 << 20 and stage["fft_pass3"] == 0.0 and stage["fft_pass2"] > 0.0
+    if fused23:                                           # the library reports the fused kernel's time as pass 2
+        stage["fft_pass23"] = stage.pop("fft_pass2")
+        stage.pop("fft_pass3")
+    fft_stages = ["fft_pass1", "fft_pass23"] if fused23 else ["fft_pass1", "fft_pass2", "fft_pass3"]
+    own_stages = ["stats", "sort", "premul", "spread", "assemble"] + (fft_stages if own_fft else [])
     dom = max(own_stages, key=lambda k: stage[k])      # the dominant OWN kernel (cuFFT, when used, is a library)
     ach = sbytes[dom] / (stage[dom] * 1e-3) / 1e9
     path_ms = stage["total"] - stage["fft"]
@@ -402,7 +409,13 @@ def run_ours(args):
         "step_ms_min": float(np.min(step_ms)), "step_ms_median": float(np.median(step_ms)),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                      "traffic": measured_traffic(dom, w, info), "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
-                     "kernel_ms": stage[dom]},
+                     "kernel_ms": stage[dom],
+                     "per_kernel": {k: {"ms": stage[k], "algorithmic_bytes": sbytes[k],
+                                        "frac": sbytes[k] / (stage[k] * 1e-3) / 1e9 / peak if stage[k] > 0 else None}
+                                    for k in own_stages},
+                     **({"note": "fft_pass23 = FFT passes 2 + 3 fused through L2: its algorithmic bytes are half of "
+                                 "the two separate passes' (the intermediate never reaches HBM); the kernel is bound "
+                                 "on the SM side (profiles/r1g_fft_l2_fusion.md)"} if fused23 else {})},
         "path_roofline": {"what": "spread + deconvolve + assembly path = all own kernels except the FFT (total - fft), "
                                   "bytes = streaming model of " + STAGE_BYTES_DOC + "; bytes_sparse = the same with the "
                                   "grid term reduced to the tiles that hold points (what the own-FFT path really writes)",
@@ -412,7 +425,9 @@ def run_ours(args):
         "fft_ms": stage["fft"],
         "fft": {"impl": "cuFFT" if ffts else "own three radix-256 passes (first pruned by the spreading kernel's "
                                              "liveness masks)" + ("; in `value` the last is fused with the assembly"
-                                                                if args.fft_impl == 2 else ""),
+                                                                if args.fft_impl == 2 else "")
+                                             + ("; passes 2 + 3 are one persistent kernel whose intermediate stays in "
+                                                "L2 and is discarded, not written back" if fused23 else ""),
                 "ms": stage["fft"], "grid_bytes": info["M"] * info["n"] * 2 * (8 if w.dtype == "f64" else 4),
                 "grid_passes_at_measured_peak": stage["fft"] * 1e-3 * peak * 1e9
                 / (2.0 * info["M"] * info["n"] * 2 * (8 if w.dtype == "f64" else 4))},

@@ -78,7 +78,7 @@ enum {
                                        which is fused with it                    */
     LS_STAGE_TOTAL = 6,         /* whole execute                                                 */
     LS_STAGE_FFT_PASS1 = 7,     /* own FFT only: the three passes, also summed into LS_STAGE_FFT  */
-    LS_STAGE_FFT_PASS2 = 8,
+    LS_STAGE_FFT_PASS2 = 8,     /*   (auto mode, n >= 2^20: the fused passes 2 + 3; PASS3 is then 0)            */
     LS_STAGE_FFT_PASS3 = 9,     /*   (pass 3 of the transforms whose modes go to the compact array) */
     LS_NUM_STAGES = 10
 };
@@ -96,11 +96,14 @@ typedef struct {
     int graph;              /* CUDA-graph replay of the execute sequence (needs timing == 0 and a non-legacy
                                stream): 0 = auto (on; off for good after three consecutive executes
                                with changed buffer pointers), 1 = never, 2 = always                 */
-    int fft_impl;           /* 0 = auto (the library's own three-pass FFT where it exists — fp64 power-of-two grids
-                               of 2^12..2^24 cells; in auto mode not for large batches of small grids — else cuFFT), 1 = cuFFT plan, 2 = own FFT with the h
-                               transforms' last pass fused with deconvolution + assembly, 3 = own FFT
-                               with the assembly as a separate kernel (what auto picks; 2 and 3 give
-                               LS_ERR_UNSUPPORTED where the own FFT does not exist)                 */
+    int fft_impl;           /* 0 = auto: the library's own FFT where it exists (fp64 power-of-two grids of
+                               2^12..2^24 cells; not for large batches of small grids), else cuFFT.  For
+                               n >= 2^20 the own FFT is a pruned first pass plus ONE persistent kernel for
+                               passes 2 + 3 whose intermediate stays in L2.  1 = cuFFT plan.  2 = own FFT,
+                               three launches, the h transforms' last pass fused with deconvolution +
+                               assembly.  3 = own FFT as three separate pass kernels and a separate
+                               assembly (same arithmetic as auto; kept for comparison).  2 and 3 give
+                               LS_ERR_UNSUPPORTED where the own FFT does not exist                   */
     int no_floating_mean;   /* 0: floating mean, six sums (default; north_star).  1: the fixed-mean form of
                                PAPER.md:17 ("four weighted trigonometric sums"): y centred by its weighted
                                mean, sinusoid model without an offset term                          */

@@ -428,6 +428,9 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     // assembly kernel (0.118 ms at 81 % of DRAM peak) plus an unfused third pass beats the fused kernel, which is
     // bound by its 2-CTAs-per-SM arithmetic, by 1 % — so fusion is opt-in (fft_impl = 2), not the default.
     p->fuse_assemble = p->own_fft && o.fft_impl == 2 && !o.dy_per_series;
+    // Passes 2 and 3 as one persistent kernel with the intermediate kept in L2 (ls_fft.cu): the default wherever
+    // the pruned three-pass transform runs; fft_impl = 3 keeps the three separate launches (for comparison).
+    p->fuse_pass23 = p->fft_prune && !p->fuse_assemble && o.fft_impl != 3;
 
     // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
     p->ndf = two_prod((double)p->n, df);
@@ -456,8 +459,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
         const size_t mask_bytes = p->fft_prune ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : 0;   // masks + 2 list counters
-        p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes;
+        const size_t queue_bytes = p->fft_prune ? (((size_t)(2 + 32 * p->slots) * 4 + 255) & ~(size_t)255) : 0;
+        p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes + queue_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
+        if (queue_bytes) p->fft_queue = (int*)((char*)p->zeroed + sums_bytes + hist_bytes + mask_bytes);
         if (p->fft_prune) {
             p->tile_counts = (int*)((char*)p->zeroed + sums_bytes + hist_bytes);
             p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes + 256);
@@ -595,6 +600,13 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 stage_begin(p, LS_STAGE_FFT_PASS1, s);
                 LS_TRY(lsb::launch_own_fft_pass1(p, ps.fft_slot0, ps.fft_batch, n_x2, s));
                 stage_end(p, s);
+                if (p->fuse_pass23) {
+                    // passes 2 + 3 in one persistent kernel, intermediate in L2 (its time is reported as pass 2)
+                    stage_begin(p, LS_STAGE_FFT_PASS2, s);
+                    LS_TRY(lsb::launch_own_fft_pass23(p, ps.fft_slot0, ps.fft_batch, s));
+                    stage_end(p, s);
+                    own += 2;
+                } else {
                 stage_begin(p, LS_STAGE_FFT_PASS2, s);
                 LS_TRY(lsb::launch_own_fft_pass2(p, ps.fft_slot0, ps.fft_batch, s));
                 stage_end(p, s);
@@ -602,6 +614,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 LS_TRY(lsb::launch_own_fft_pass3(p, ps.fft_slot0, n_modes, s));
                 stage_end(p, s);
                 own += 1 + (p->n > 65536 ? 1 : 0) + (n_modes > 0 ? 1 : 0);
+                }
             } else {
                 stage_begin(p, LS_STAGE_FFT, s);
                 cufftHandle h = find_fft(p, ps.fft_batch);

@@ -358,6 +358,143 @@ ls_fft_rows_kernel(const FftArgs a) {
     }
 }
 
+// Passes 2 + 3 as ONE persistent kernel that keeps the intermediate in L2 (n >= 2^20, unfused assembly).
+// After pass 1 the problem is R1 independent 65536-point transforms (row k1 = 1 MB, contiguous).  A SLAB is the C = 8
+// rows k1 = C g .. C g + C - 1 of one transform (8 MB): pass 2 on it is 256 tiles (C rows x 256 / C column tiles),
+// pass 3 on it is 256 tiles (one per k2, C consecutive k1 each — the unit that stores runs of C consecutive
+// frequencies, 128 bytes).  CTAs (128 threads, four per SM) draw tiles from an ordered queue
+//   [pass 2 of slab b][pass 3 of slab b - lag],  b = 0, 1, ...
+// and a pass-3 tile first waits until all 256 pass-2 tiles of its slab have been signalled done.  Every tile a CTA
+// can wait for was drawn earlier, by a CTA that is running and never waits before it signals, so the queue cannot
+// deadlock.  What a slab's pass 2 writes is read back by its pass 3 a few microseconds later out of the 126 MB L2
+// (ncu: 0.02 % of pass 3's input comes from DRAM), and once read the lines are dead: `discard.global.L2` drops them
+// before they are ever written back.  DRAM traffic of the two passes: 3.0 GB -> 1.48 GB at config 3
+// (profiles/r1g_fft_l2_fusion.md).  lag = 2: one slab is less than half a wave of the 592 resident CTAs.
+// After the kernel the fine grids hold indeterminate values; nothing reads them again (the next execute's spreading
+// kernel rewrites every tile that pass 1 will load).
+// queue: [0] next item, [1] CTAs that left, [2 + s] pass-2 tiles of slab s done.  The last CTA to leave zeroes it.
+constexpr int kC23 = 8;                  // tile width of the fused kernel
+constexpr int kLag23 = 2;
+template <int C>                                          // C columns (pass 2) / rows (pass 3) per tile, 16 C threads
+__global__ void __launch_bounds__(16 * C, 512 / (16 * C))
+ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
+    constexpr int lag = kLag23;
+    constexpr int T = 16 * C, CT = 256 / C;                  // threads; column tiles per row
+    extern __shared__ __align__(16) unsigned char fsm[];
+    double2* Y = reinterpret_cast<double2*>(fsm);            // pass 2: [ka][j][C]; pass 3: [ka][j][C + 1]
+    double2* w256 = Y + 256 * (C + 1);
+    __shared__ int s_item;
+    for (int i = threadIdx.x; i < 256; i += T) {
+        double sn, cs;
+        sincospi((double)i / 128.0, &sn, &cs);
+        w256[i] = make_double2(cs, sn);
+    }
+    const int groups = a.R1 / C;                             // slabs per transform
+    const int total = (nslabs + lag) * 512;
+    if (threadIdx.x == 0) s_item = atomicAdd(&queue[0], 1);
+    for (;;) {
+        __syncthreads();                                     // s_item written; (first time) w256 ready
+        const int item = s_item;
+        if (item >= total) break;
+        // the next draw is requested now and parked in a register: its latency hides behind this tile
+        int next_item = 0;
+        if (threadIdx.x == 0) next_item = atomicAdd(&queue[0], 1);
+        const int b = item >> 9, slot = item & 255;
+        double2 x[16];
+        if ((item & 256) == 0) {
+            // ---- pass 2 tile: row k1 = C g + slot / CT, columns C (slot % CT) ..
+            if (b >= nslabs) goto next;
+            const int tr = b / groups, g = b - tr * groups;
+            const int k1 = C * g + slot / CT;
+            const int c = threadIdx.x % C, hi4 = threadIdx.x / C;
+            const long long m = (long long)(slot % CT) * C + c;
+            double2* base = a.grids + (long long)tr * a.n + (long long)k1 * 65536 + m;
+            {
+                const int j = hi4;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = base[(long long)(16 * i + j) * 256];
+                fft16(x);
+#pragma unroll
+                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * C + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+            }
+            __syncthreads();
+            {
+                const int ka = hi4;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * C + c];
+                fft16(x);
+                const unsigned mm = (unsigned)m * (unsigned)a.R1;
+                double2 tw = twiddle_n(a, (unsigned)ka * mm);
+                const double2 st = twiddle_n(a, 16u * mm);
+#pragma unroll
+                for (int kb = 0; kb < 16; ++kb) {
+                    base[(long long)(ka + 16 * kb) * 256] = cmul(x[pos16(kb)], tw);
+                    tw = cmul(tw, st);
+                }
+            }
+            __syncthreads();                                 // every thread's stores are issued ...
+            if (threadIdx.x == 0) {
+                __threadfence();                             // ... and ordered before the signal, device-wide
+                atomicAdd(&queue[2 + b], 1);
+            }
+        } else {
+            // ---- pass 3 tile: k2 = slot, k1 = C g .. C g + C - 1
+            const int sl = b - lag;
+            if (sl < 0) goto next;
+            const int tr = sl / groups, g = sl - tr * groups;
+            if (threadIdx.x == 0) {
+                const volatile int* done = queue + 2 + sl;
+                while (*done < 256) __nanosleep(40);
+                __threadfence();
+            }
+            __syncthreads();
+            const int rho_b = slot * a.R1 + C * g;
+            const double2* src = a.grids + (long long)tr * a.n;
+            {
+                const int j = threadIdx.x & 15, c = threadIdx.x >> 4;
+                const double2* row = src + ((long long)(C * g + c) * 256 + slot) * 256;
+#pragma unroll
+                for (int i = 0; i < 16; ++i) x[i] = __ldcg(&row[16 * i + j]);    // written by other SMs: read at L2
+                fft16(x);
+#pragma unroll
+                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+            }
+            __syncthreads();
+            {
+                // the slab is dead once read: drop its dirty lines from L2 instead of writing them back to HBM
+                // (thread (c, j) drops lines 2 j and 2 j + 1 of row c's 4 KB chunk; all its loads have landed)
+                const int j = threadIdx.x & 15, c = threadIdx.x >> 4;
+                const double2* row = src + ((long long)(C * g + c) * 256 + slot) * 256 + 16 * j;
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(row) : "memory");
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(row + 8) : "memory");
+            }
+            {
+                const int c = threadIdx.x % C, ka = threadIdx.x / C;
+#pragma unroll
+                for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * (C + 1) + c];
+                fft16(x);
+                double2* out = a.modes + (long long)tr * a.Nf;
+                const long long kk0 = rho_b + c;
+                const long long r12 = (long long)a.R1 * 256;
+#pragma unroll
+                for (int kb = 0; kb < 16; ++kb) {
+                    long long k = kk0 + r12 * (ka + 16 * kb) + a.half;
+                    if (k >= a.n) k -= a.n;
+                    if (k < a.Nf) out[k] = x[pos16(kb)];
+                }
+            }
+        }
+    next:
+        __syncthreads();                                     // Y is free and everybody has read s_item
+        if (threadIdx.x == 0) s_item = next_item;
+    }
+    if (threadIdx.x == 0) {
+        if (atomicAdd(&queue[1], 1) == (int)gridDim.x - 1) {  // last CTA out: nobody draws or waits any more
+            for (int i = 0; i < nslabs + 2; ++i) queue[i] = 0;
+        }
+    }
+}
+
 __global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < 4096) {
@@ -374,6 +511,7 @@ __global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
 
 constexpr size_t kColsSmem = sizeof(double2) * (256 * kC + 256);
 constexpr size_t kRowsSmem = sizeof(double2) * (256 * (kC + 1) + 256);
+constexpr size_t k23Smem = sizeof(double2) * (256 * (kC23 + 1) + 256);
 
 }  // namespace
 
@@ -402,6 +540,8 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<kC23>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     return cudaFuncSetAttribute(ls_fft_rows_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem);
@@ -466,6 +606,17 @@ cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream
     if (a.R2 == 1) return cudaSuccess;                     // two-pass sizes: nothing between pass 1 and the last pass
     dim3 g2(256 / kC, a.R1, ntrans);                       // [k1][l2][l3]: outer = R1 blocks, stride 256
     ls_fft_cols_kernel<<<g2, kFftThreads, kColsSmem, s>>>(a, a.R1, 256);
+    return cudaGetLastError();
+}
+
+// Passes 2 and 3 of transforms [slot0, slot0 + ntrans) in one persistent kernel (n >= 2^20): compact modes out,
+// fine grids left indeterminate.
+cudaError_t launch_own_fft_pass23(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
+    FftArgs a;
+    fill_common(p, a, slot0, 0);
+    const int nslabs = ntrans * (a.R1 / kC23);
+    const int nblk = std::min(nslabs * 256, (512 / (16 * kC23)) * p->num_sms);
+    ls_fft_pass23_kernel<kC23><<<nblk, 16 * kC23, k23Smem, s>>>(a, nslabs, p->fft_queue);
     return cudaGetLastError();
 }
 

@@ -113,10 +113,12 @@ struct ls_plan_s {
     bool own_fft = false;
     bool fft_prune = false;                         // spreading skips empty tiles, FFT pass 1 prunes by liveness masks
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
+    bool fuse_pass23 = false;                      // FFT passes 2 + 3 as one persistent kernel (intermediate in L2)
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
     void* modes = nullptr;                          // [slots][Nf] complex: kept modes in frequency order
     int* tile_list = nullptr;                       // [2][ntiles] occupied spreading tiles per point set (x2, x1)
     int* tile_counts = nullptr;                     // [2] list lengths (in `zeroed`)
+    int* fft_queue = nullptr;                       // [2 + 16 slots] work queue of the fused FFT passes 2 + 3 (in `zeroed`)
     unsigned* row_masks = nullptr;                  // [2][65536/L][<=16] liveness bits for FFT pass 1 (in `zeroed`)
     // CUDA-graph replay of the execute sequence (launch-latency-bound small problems; opts.graph)
     bool use_graph = false;
@@ -155,6 +157,7 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s);
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
 cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
+cudaError_t launch_own_fft_pass23(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
 cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int series0, int w_slot, int w2_slot,
                                     void* power, cudaStream_t s);
 // ---- ls_post.cu: P0 table, K5+K6 -----------------------------------------------------------

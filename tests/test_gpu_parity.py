@@ -125,6 +125,32 @@ def test_own_fft_other_power_of_two_grids(p):
     assert int(np.argmax(P_own[0])) == kg
 
 
+@pytest.mark.parametrize("p,batch", [(20, 1), (21, 3), (22, 1), (23, 2)])
+def test_own_fft_fused_passes_match_separate_passes(p, batch):
+    """n = 2^p >= 2^20, default plan: FFT passes 2 + 3 run as one persistent kernel whose intermediate stays in L2
+    (tile queue, slab completion signals, L2 discard).  Same arithmetic as the three separate pass kernels
+    (fft_impl = 3), so the powers must agree to rounding — also on replays (the queue resets itself) — and match the
+    oracle on sampled k."""
+    rng = np.random.default_rng(900 + p)
+    Nf = int(0.7 * (1 << p))
+    Nd = max(500, Nf // 10)
+    t = rng.uniform(0, 3000.0, Nd)
+    dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    kg = Nf // 4
+    y = np.stack([np.sin(2 * np.pi * (df + (kg + 10 * b) * df) * t + 0.3 * b) + rng.normal(0, 1.0, Nd) for b in range(batch)])
+    w = Workload(f"fused23_p{p}", t, y, dy, df, df, Nf, "f64", 1e-9)
+    P_f, ex = gpu_power(w, no_autotune=1, return_plan_info=True, side_stream=True, repeat=3)
+    assert ex["info"]["n"] == 1 << p and ex["launches"][1] == 0
+    P_s, ex_s = gpu_power(w, no_autotune=1, fft_impl=3, return_plan_info=True)
+    assert ex_s["launches"][0] == ex["launches"][0] + 1                 # one launch fewer than the separate passes
+    assert np.max(np.abs(P_f - P_s)) <= 1e-13                           # (the statistics' atomic sums are unordered)
+    ks = np.unique(np.concatenate([compare_indices(w, 150), np.arange(kg - 3, kg + 4)]))
+    for b in range(batch):
+        wb = Workload(w.name, t, np.ascontiguousarray(y[b:b + 1]), dy, df, df, Nf, "f64", 1e-9)
+        _check64(errors(P_f[b][ks], oracle_power(wb, ks=ks)))
+
+
 def test_own_fft_per_series_dy_and_dense_points():
     """Own FFT (n = 2^20) with per-series dy (slots [w2_s ...][(w_s, h_s) ...], liveness masks of both point sets) and
     more points than a spreading chunk holds per tile (several 256-candidate chunks per tile)."""
