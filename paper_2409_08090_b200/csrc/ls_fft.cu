@@ -134,8 +134,20 @@ __device__ __forceinline__ double2 twiddle_n(const FftArgs& a, unsigned e) {
     return cmul(lo, hi);
 }
 
-// w_256^m table in shared memory
-__device__ __forceinline__ void fill_w256(double2* w256) {
+// Exchange twiddles in shared memory, stored as [ka][j] = w_256^{j ka} (j, ka < 16) rather than as a w_256^m table:
+// the threads of a warp that differ in j read consecutive entries (no bank conflicts; with an m-indexed table the
+// lookups of ka = 8 were 16-way conflicts in pass 3), threads that share j read the same entry (broadcast).
+// Passes 2 + 3 at config 3: 0.441 -> 0.430 ms.
+__device__ __forceinline__ void fill_w256(double2* w256, int nthreads = kFftThreads) {
+    for (int i = threadIdx.x; i < 256; i += nthreads) {
+        double s, c;
+        sincospi((double)((i >> 4) * (i & 15)) / 128.0, &s, &c);
+        w256[i] = make_double2(c, s);
+    }
+}
+// the plain table w_256^m, m < 256 (pass 1: two values of j per warp, nothing to gain from the layout above; measured
+// 2 % slower with it)
+__device__ __forceinline__ void fill_w256_linear(double2* w256) {
     for (int i = threadIdx.x; i < 256; i += kFftThreads) {
         double s, c;
         sincospi((double)i / 128.0, &s, &c);
@@ -164,7 +176,7 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
         fft16(x);
         __syncthreads();                                     // w256 ready
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
     }
     __syncthreads();
     {
@@ -197,7 +209,7 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
     double2* w256 = Y + 4096;
-    fill_w256(w256);
+    fill_w256_linear(w256);
     const int c = threadIdx.x % C, hi = threadIdx.x / C;     // hi: j in stage 1, item group in stage 2
     auto mask_of = [&](int tile) -> unsigned {
         if (tile >= ntiles_total) return 0u;
@@ -300,7 +312,7 @@ ls_fft_rows_kernel(const FftArgs a) {
         fft16(x);
         __syncthreads();
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (kC + 1) + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (kC + 1) + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
     }
     __syncthreads();
     {
@@ -375,6 +387,7 @@ ls_fft_rows_kernel(const FftArgs a) {
 // queue: [0] next item, [1] CTAs that left, [2 + s] pass-2 tiles of slab s done.  The last CTA to leave zeroes it.
 constexpr int kC23 = 8;                  // tile width of the fused kernel
 constexpr int kLag23 = 2;
+constexpr int kPrefetch23 = 512;             // queue distance of the L2 prefetch: the same tile of the next slab
 template <int C>                                          // C columns (pass 2) / rows (pass 3) per tile, 16 C threads
 __global__ void __launch_bounds__(16 * C, 512 / (16 * C))
 ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
@@ -384,11 +397,7 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
     double2* Y = reinterpret_cast<double2*>(fsm);            // pass 2: [ka][j][C]; pass 3: [ka][j][C + 1]
     double2* w256 = Y + 256 * (C + 1);
     __shared__ int s_item;
-    for (int i = threadIdx.x; i < 256; i += T) {
-        double sn, cs;
-        sincospi((double)i / 128.0, &sn, &cs);
-        w256[i] = make_double2(cs, sn);
-    }
+    fill_w256(w256, T);
     const int groups = a.R1 / C;                             // slabs per transform
     const int total = (nslabs + lag) * 512;
     if (threadIdx.x == 0) s_item = atomicAdd(&queue[0], 1);
@@ -413,9 +422,22 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 const int j = hi4;
 #pragma unroll
                 for (int i = 0; i < 16; ++i) x[i] = base[(long long)(16 * i + j) * 256];
+                {
+                    // pull the pass-2 tile one slab further down the queue (some CTA draws it about a wave from now)
+                    // from HBM into L2: its loads then wait for L2, not for DRAM (0.450 -> 0.441 ms at config 3)
+                    const int it = item + kPrefetch23;
+                    const int pb = it >> 9, ps = it & 255;
+                    if (pb < nslabs) {
+                        const int ptr = pb / groups, pg = pb - ptr * groups;
+                        const double2* pbase = a.grids + (long long)ptr * a.n + (long long)(C * pg + ps / CT) * 65536 +
+                                               (long long)(ps % CT) * C;
+                        for (int r = threadIdx.x; r < 256; r += T)      // one 128-byte line per row of the tile
+                            asm volatile("prefetch.global.L2 [%0];" ::"l"(pbase + (long long)r * 256));
+                    }
+                }
                 fft16(x);
 #pragma unroll
-                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * C + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * C + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
             }
             __syncthreads();
             {
@@ -457,7 +479,7 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 for (int i = 0; i < 16; ++i) x[i] = __ldcg(&row[16 * i + j]);    // written by other SMs: read at L2
                 fft16(x);
 #pragma unroll
-                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], w256[(j * ka) & 255]);
+                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
             }
             __syncthreads();
             {
