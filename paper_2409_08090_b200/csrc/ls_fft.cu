@@ -398,6 +398,10 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
     double2* w256 = Y + 256 * (C + 1);
     __shared__ int s_item;
     fill_w256(w256, T);
+    // w_256^{16 j} = e^{2 pi i j / 16} for this thread's j in a pass-2 tile (j = tid / C) and in a pass-3 tile (j = tid % 16)
+    double2 c16_p2, c16_p3;
+    sincospi((double)(threadIdx.x / C) / 8.0, &c16_p2.y, &c16_p2.x);
+    sincospi((double)(threadIdx.x & 15) / 8.0, &c16_p3.y, &c16_p3.x);
     const int groups = a.R1 / C;                             // slabs per transform
     const int total = (nslabs + lag) * 512;
     if (threadIdx.x == 0) s_item = atomicAdd(&queue[0], 1);
@@ -437,7 +441,14 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 }
                 fft16(x);
 #pragma unroll
-                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * C + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
+                for (int ka = 0; ka <= 8; ++ka) {
+                    // w^{j ka} from the table for ka <= 8; w^{j (16 - ka)} = w^{16 j} conj(w^{j ka}) (one multiplication
+                    // by a per-thread constant instead of a shared-memory lookup: the kernel is LSU-bound)
+                    if (ka == 0) { Y[j * C + c] = x[0]; continue; }
+                    const double2 t = w256[ka * 16 + j];
+                    Y[(ka * 16 + j) * C + c] = cmul(x[pos16(ka)], t);
+                    if (ka < 8) Y[((16 - ka) * 16 + j) * C + c] = cmul(cmul(x[pos16(16 - ka)], c16_p2), make_double2(t.x, -t.y));
+                }
             }
             __syncthreads();
             {
@@ -479,7 +490,12 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 for (int i = 0; i < 16; ++i) x[i] = __ldcg(&row[16 * i + j]);    // written by other SMs: read at L2
                 fft16(x);
 #pragma unroll
-                for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
+                for (int ka = 0; ka <= 8; ++ka) {
+                    if (ka == 0) { Y[j * (C + 1) + c] = x[0]; continue; }
+                    const double2 t = w256[ka * 16 + j];
+                    Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], t);
+                    if (ka < 8) Y[((16 - ka) * 16 + j) * (C + 1) + c] = cmul(cmul(x[pos16(16 - ka)], c16_p3), make_double2(t.x, -t.y));
+                }
             }
             __syncthreads();
             {
