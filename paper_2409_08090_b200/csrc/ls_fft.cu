@@ -396,7 +396,7 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // pass 2: [ka][j][C]; pass 3: [ka][j][C + 1]
     double2* w256 = Y + 256 * (C + 1);
-    __shared__ int s_item;
+    __shared__ int s_item[2];                                // the CTA's current / next queue item (double-buffered)
     fill_w256(w256, T);
     // w_256^{16 j} = e^{2 pi i j / 16} for this thread's j in a pass-2 tile (j = tid / C) and in a pass-3 tile (j = tid % 16)
     double2 c16_p2, c16_p3;
@@ -404,10 +404,12 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
     sincospi((double)(threadIdx.x & 15) / 8.0, &c16_p3.y, &c16_p3.x);
     const int groups = a.R1 / C;                             // slabs per transform
     const int total = (nslabs + lag) * 512;
-    if (threadIdx.x == 0) s_item = atomicAdd(&queue[0], 1);
-    for (;;) {
-        __syncthreads();                                     // s_item written; (first time) w256 ready
-        const int item = s_item;
+    if (threadIdx.x == 0) s_item[0] = atomicAdd(&queue[0], 1);
+    __syncthreads();                                         // s_item[0], w256 ready
+    // Barriers per tile: the exchange and ONE more that frees Y, publishes the next item (written by thread 0 into the
+    // other half of s_item just before it) and, for a pass-2 tile, certifies that every thread's stores are issued.
+    for (int par = 0;; par ^= 1) {
+        const int item = s_item[par];
         if (item >= total) break;
         // the next draw is requested now and parked in a register: its latency hides behind this tile
         int next_item = 0;
@@ -465,11 +467,13 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                     tw = cmul(tw, st);
                 }
             }
+            if (threadIdx.x == 0) s_item[par ^ 1] = next_item;
             __syncthreads();                                 // every thread's stores are issued ...
             if (threadIdx.x == 0) {
                 __threadfence();                             // ... and ordered before the signal, device-wide
                 atomicAdd(&queue[2 + b], 1);
             }
+            continue;
         } else {
             // ---- pass 3 tile: k2 = slot, k1 = C g .. C g + C - 1
             const int sl = b - lag;
@@ -510,6 +514,8 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 const int c = threadIdx.x % C, ka = threadIdx.x / C;
 #pragma unroll
                 for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * (C + 1) + c];
+                if (threadIdx.x == 0) s_item[par ^ 1] = next_item;
+                __syncthreads();                             // Y is free
                 fft16(x);
                 double2* out = a.modes + (long long)tr * a.Nf;
                 const long long kk0 = rho_b + c;
@@ -521,10 +527,11 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                     if (k < a.Nf) out[k] = x[pos16(kb)];
                 }
             }
+            continue;
         }
-    next:
-        __syncthreads();                                     // Y is free and everybody has read s_item
-        if (threadIdx.x == 0) s_item = next_item;
+    next:                                                    // items past either end of the slab sequence: nothing to do
+        if (threadIdx.x == 0) s_item[par ^ 1] = next_item;
+        __syncthreads();
     }
     if (threadIdx.x == 0) {
         if (atomicAdd(&queue[1], 1) == (int)gridDim.x - 1) {  // last CTA out: nobody draws or waits any more
