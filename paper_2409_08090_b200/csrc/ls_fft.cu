@@ -16,7 +16,8 @@
 //     df = 1/(5T)), and the spreading kernel no longer has to write those zeros;
 //   * pass 3 writes only the N_f kept modes, already centred, so the assembly reads a dense array.
 //
-// One CTA = 256 threads = one tile of 256 (transform dimension) x 16 (other dimension) points:
+// One CTA = 256 threads = one tile of 256 (transform dimension) x 16 (other dimension) points (pass 1 and the fused
+// passes 2 + 3: 128 threads, 256 x 8):
 // 16-point FFTs in registers (radix 4 x 4), one shared-memory exchange (conflict-free layouts),
 // 256-byte global segments on both sides.  Twiddles: w_256 from a shared table, w_n^e from two
 // 4096-entry tables (e = 4096 e_hi + e_lo) and a base/step recurrence along the thread's 16 outputs.
@@ -147,8 +148,8 @@ __device__ __forceinline__ void fill_w256(double2* w256, int nthreads = kFftThre
 }
 // the plain table w_256^m, m < 256 (pass 1: two values of j per warp, nothing to gain from the layout above; measured
 // 2 % slower with it)
-__device__ __forceinline__ void fill_w256_linear(double2* w256) {
-    for (int i = threadIdx.x; i < 256; i += kFftThreads) {
+__device__ __forceinline__ void fill_w256_linear(double2* w256, int nthreads) {
+    for (int i = threadIdx.x; i < 256; i += nthreads) {
         double s, c;
         sincospi((double)i / 128.0, &s, &c);
         w256[i] = make_double2(c, s);
@@ -197,19 +198,18 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
     }
 }
 
-// Pass 1, pruned and persistent: radix R1 = 16 RB over l1 (row stride inner = 65536 cells), C = 256 / RB
-// columns per tile, so a tile is always 4096 points = 256 threads x 16.  Stage 1: 16-point FFTs over i (rows
+// Pass 1, pruned and persistent: radix R1 = 16 RB over l1 (row stride inner = 65536 cells), C = T / RB
+// columns per tile, so a tile is always 16 T points (T = 128 threads: 2048 points, four CTAs per SM).  Stage 1: 16-point FFTs over i (rows
 // RB i + j); stage 2: RB-point FFTs over j.  The 16-bit liveness mask of the NEXT tile is fetched while the
 // current one is in flight, so it never sits on the critical path; dead rows are not loaded (never written).
-template <int RB>
-__global__ void __launch_bounds__(kFftThreads, 512 / kFftThreads)
+template <int RB, int T>
+__global__ void __launch_bounds__(T, 512 / T)
 ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int ntiles_total) {
-    constexpr int C = 256 / RB, NI = 16 / RB, TWS = 16 / RB;   // TWS: stride of w_{R1} in the w_256 table
-    static_assert(kFftThreads == 256, "pass 1 is written for 256 threads");
+    constexpr int C = T / RB, NI = 16 / RB, TWS = 16 / RB;     // TWS: stride of w_{R1} in the w_256 table
     extern __shared__ __align__(16) unsigned char fsm[];
     double2* Y = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
-    double2* w256 = Y + 4096;
-    fill_w256_linear(w256);
+    double2* w256 = Y + 16 * T;
+    fill_w256_linear(w256, T);
     const int c = threadIdx.x % C, hi = threadIdx.x / C;     // hi: j in stage 1, item group in stage 2
     auto mask_of = [&](int tile) -> unsigned {
         if (tile >= ntiles_total) return 0u;
@@ -555,6 +555,8 @@ __global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
 }
 
 constexpr size_t kColsSmem = sizeof(double2) * (256 * kC + 256);
+constexpr int kPass1Threads = 128;
+constexpr size_t kPass1Smem = sizeof(double2) * (16 * kPass1Threads + 256);
 constexpr size_t kRowsSmem = sizeof(double2) * (256 * (kC + 1) + 256);
 constexpr size_t k23Smem = sizeof(double2) * (256 * (kC23 + 1) + 256);
 
@@ -579,11 +581,11 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     ls_fft_tables_kernel<<<(cnt + 255) / 256, 256, 0, s>>>((double2*)p->fft_wlo, (double2*)p->fft_whi, p->n);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<16, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<8, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<4, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<2, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<kC23>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
@@ -633,14 +635,17 @@ cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, 
         return cudaGetLastError();
     }
     const int rb = own_fft_rb(p);
-    const int tiles_per_trans = (int)(inner1 / (256 / rb)), total = tiles_per_trans * ntrans;
-    const int nblk = std::min(total, (512 / kFftThreads) * p->num_sms);
+    // 128-thread CTAs (tiles of 2048 points, four CTAs per SM): a barrier then waits for four warps, not eight
+    // (pass 1 at config 3: 0.215 -> 0.207 ms against 256-thread CTAs with 4096-point tiles)
+    constexpr int T = kPass1Threads;
+    const int tiles_per_trans = (int)(inner1 / (T / rb)), total = tiles_per_trans * ntrans;
+    const int nblk = std::min(total, (512 / T) * p->num_sms);
     switch (rb) {
-        case 16: ls_fft_pass1_kernel<16><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
-        case 8: ls_fft_pass1_kernel<8><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
-        case 4: ls_fft_pass1_kernel<4><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
-        case 2: ls_fft_pass1_kernel<2><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
-        default: ls_fft_pass1_kernel<1><<<nblk, kFftThreads, kColsSmem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 16: ls_fft_pass1_kernel<16, T><<<nblk, T, kPass1Smem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 8: ls_fft_pass1_kernel<8, T><<<nblk, T, kPass1Smem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 4: ls_fft_pass1_kernel<4, T><<<nblk, T, kPass1Smem, s>>>(a, inner1, tiles_per_trans, total); break;
+        case 2: ls_fft_pass1_kernel<2, T><<<nblk, T, kPass1Smem, s>>>(a, inner1, tiles_per_trans, total); break;
+        default: ls_fft_pass1_kernel<1, T><<<nblk, T, kPass1Smem, s>>>(a, inner1, tiles_per_trans, total); break;
     }
     return cudaGetLastError();
 }
