@@ -292,6 +292,7 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
         return c;
     };
     int tile_cur = 0, tile_nx = 0;
+    bool cnt_clean = false;
     Cand cand_cur{0, 0, 0, 0, 0, 0};
     if (a.skip_empty) {
         tile_cur = item_tile(blockIdx.x);
@@ -363,9 +364,10 @@ ls_spread_tile_kernel(const __grid_constant__ SpreadArgs<T> a) {
                 have = rel + w > 0 && rel < Lt;
             }
         }
-        if (base == 0) {                             // later chunks find cnt re-zeroed by the scan
-            for (int i = threadIdx.x; i < HN; i += kSpreadThreads) cnt[i] = 0;
+        if (!cnt_clean) {                            // later chunks, and later tiles of a persistent CTA, find cnt
+            for (int i = threadIdx.x; i < HN; i += kSpreadThreads) cnt[i] = 0;   // re-zeroed by the scan
             __syncthreads();
+            cnt_clean = true;
         }
         // key = first-touched cell + (w - 1); rank = arrival order among equal keys
         const int key = rel + w - 1;
