@@ -135,6 +135,33 @@ __device__ __forceinline__ double2 twiddle_n(const FftArgs& a, unsigned e) {
     return cmul(lo, hi);
 }
 
+// Second-stage outputs k_r = ka + 16 kb, kb < NOUT, times the inter-pass twiddle tw st^kb, stored `stride` cells apart.
+// For NOUT = 16 the twiddles come from TWO interleaved recurrences (even / odd kb, step st^2): these kernels are latency-bound, and
+// a single chain of NOUT dependent complex products is what the stores end up waiting for (fused passes 2 + 3 at
+// config 3: 0.416 -> 0.407 ms; four chains spill at the 128-register cap: 0.425 ms).
+template <int NOUT, typename Get>
+__device__ __forceinline__ void store_twiddled(double2* base, long long stride, int ka, double2 tw, double2 st, Get get) {
+    if constexpr (NOUT == 16) {                              // shorter chains keep the single recurrence
+        double2 tw1 = cmul(tw, st);
+        const double2 st2 = cmul(st, st);
+#pragma unroll
+        for (int kb = 0; kb < NOUT; kb += 2) {
+            base[(long long)(ka + 16 * kb) * stride] = cmul(get(kb), tw);
+            base[(long long)(ka + 16 * kb + 16) * stride] = cmul(get(kb + 1), tw1);
+            if (kb + 2 < NOUT) {
+                tw = cmul(tw, st2);
+                tw1 = cmul(tw1, st2);
+            }
+        }
+    } else {
+#pragma unroll
+        for (int kb = 0; kb < NOUT; ++kb) {
+            base[(long long)(ka + 16 * kb) * stride] = cmul(get(kb), tw);
+            tw = cmul(tw, st);
+        }
+    }
+}
+
 // Exchange twiddles in shared memory, stored as [ka][j] = w_256^{j ka} (j, ka < 16) rather than as a w_256^m table:
 // the threads of a warp that differ in j read consecutive entries (no bank conflicts; with an m-indexed table the
 // lookups of ka = 8 were 16-way conflicts in pass 3), threads that share j read the same entry (broadcast).
@@ -188,13 +215,9 @@ ls_fft_cols_kernel(const FftArgs a, int outer, long long inner) {
         // k_r = ka + 16 kb;  twiddle exponent e = k_r * m * outer (mod n) = e0 + kb * de
         // (requesting the tables before the exchange, as pass 1 does, costs this DRAM-bound pass registers: slower)
         const unsigned mm = (unsigned)m * (unsigned)outer;
-        double2 tw = twiddle_n(a, (unsigned)ka * mm);
+        const double2 tw = twiddle_n(a, (unsigned)ka * mm);
         const double2 st = twiddle_n(a, 16u * mm);
-#pragma unroll
-        for (int kb = 0; kb < 16; ++kb) {
-            base[(long long)(ka + 16 * kb) * inner] = cmul(x[pos16(kb)], tw);
-            tw = cmul(tw, st);
-        }
+        store_twiddled<16>(base, inner, ka, tw, st, [&](int kb) { return x[pos16(kb)]; });
     }
 }
 
@@ -254,12 +277,8 @@ ls_fft_pass1_kernel(const FftArgs a, long long inner, int tiles_per_trans, int n
                 for (int j = 0; j < RB; ++j) y[j] = Y[(ka * RB + j) * C + c];
                 fft_small<RB>(y);
                 // k1 = ka + 16 kb;  twiddle exponent k1 * m = ka m + kb (16 m)
-                double2 tw = q == 0 ? tw0 : twiddle_n(a, (unsigned)ka * mm);
-#pragma unroll
-                for (int kb = 0; kb < RB; ++kb) {
-                    base[(long long)(ka + 16 * kb) * inner] = cmul(y[fft_pos<RB>(kb)], tw);
-                    tw = cmul(tw, st);
-                }
+                const double2 tw = q == 0 ? tw0 : twiddle_n(a, (unsigned)ka * mm);
+                store_twiddled<RB>(base, inner, ka, tw, st, [&](int kb) { return y[fft_pos<RB>(kb)]; });
             }
         }
         __syncthreads();                                     // Y is reused by the next tile
@@ -459,13 +478,9 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * C + c];
                 fft16(x);
                 const unsigned mm = (unsigned)m * (unsigned)a.R1;
-                double2 tw = twiddle_n(a, (unsigned)ka * mm);
+                const double2 tw = twiddle_n(a, (unsigned)ka * mm);
                 const double2 st = twiddle_n(a, 16u * mm);
-#pragma unroll
-                for (int kb = 0; kb < 16; ++kb) {
-                    base[(long long)(ka + 16 * kb) * 256] = cmul(x[pos16(kb)], tw);
-                    tw = cmul(tw, st);
-                }
+                store_twiddled<16>(base, 256, ka, tw, st, [&](int kb) { return x[pos16(kb)]; });
             }
             if (threadIdx.x == 0) s_item[par ^ 1] = next_item;
             __syncthreads();                                 // every thread's stores are issued ...
@@ -524,7 +539,7 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
                 for (int kb = 0; kb < 16; ++kb) {
                     long long k = kk0 + r12 * (ka + 16 * kb) + a.half;
                     if (k >= a.n) k -= a.n;
-                    if (k < a.Nf) out[k] = x[pos16(kb)];
+                    if (k < a.Nf) __stcs(&out[k], x[pos16(kb)]);     // read once, by the assembly, after 600 MB more
                 }
             }
             continue;
