@@ -406,6 +406,11 @@ ls_fft_rows_kernel(const FftArgs a) {
 // queue: [0] next item, [1] CTAs that left, [2 + s] pass-2 tiles of slab s done.  The last CTA to leave zeroes it.
 constexpr int kC23 = 8;                  // tile width of the fused kernel
 constexpr int kLag23 = 2;
+__device__ __forceinline__ int ld_acquire_gpu(const int* p) {
+    int v;
+    asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 constexpr int kPrefetch23 = 512;             // queue distance of the L2 prefetch: the same tile of the next slab
 template <int C>                                          // C columns (pass 2) / rows (pass 3) per tile, 16 C threads
 __global__ void __launch_bounds__(16 * C, 512 / (16 * C))
@@ -485,8 +490,9 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
             if (threadIdx.x == 0) s_item[par ^ 1] = next_item;
             __syncthreads();                                 // every thread's stores are issued ...
             if (threadIdx.x == 0) {
-                __threadfence();                             // ... and ordered before the signal, device-wide
-                atomicAdd(&queue[2 + b], 1);
+                // ... and ordered before the signal, device-wide: a release reduction (MEMBAR.ALL.GPU) instead of
+                // __threadfence() + atomicAdd (MEMBAR.SC.GPU): 0.4005 -> 0.396 ms
+                asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(queue + 2 + b) : "memory");
             }
             continue;
         } else {
@@ -495,9 +501,10 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
             if (sl < 0) goto next;
             const int tr = sl / groups, g = sl - tr * groups;
             if (threadIdx.x == 0) {
-                const volatile int* done = queue + 2 + sl;
-                while (*done < 256) __nanosleep(40);
-                __threadfence();
+                // acquire load, not volatile load + __threadfence(): the fence would also wait for this thread's own
+                // stores of the previous tile to drain, with the whole CTA parked at the barrier below (0.406 -> 0.4005 ms)
+                const int* done = queue + 2 + sl;
+                while (ld_acquire_gpu(done) < 256) __nanosleep(40);
             }
             __syncthreads();
             const int rho_b = slot * a.R1 + C * g;
