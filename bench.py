@@ -253,9 +253,9 @@ def stage_model_bytes(w, info, own_fft, L):
 
 def measured_traffic(kernel_stage, w, info):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    ncu --set full capture (profiles/r1i_traffic.csv; same command line, config 3 defaults).  None when
+    ncu --set full capture (profiles/r1j_traffic.csv; same command line, config 3 defaults).  None when
     the capture does not cover this workload / plan."""
-    path = os.path.join(ROOT, "profiles", "r1i_traffic.csv")
+    path = os.path.join(ROOT, "profiles", "r1j_traffic.csv")
     try:
         with open(path) as f:
             rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
@@ -415,7 +415,7 @@ def run_ours(args):
                                     for k in own_stages},
                      **({"note": "fft_pass23 = FFT passes 2 + 3 fused through L2: its algorithmic bytes are half of "
                                  "the two separate passes' (the intermediate never reaches HBM); the kernel is bound "
-                                 "on the SM side (profiles/r1i_cfg3.md)"} if fused23 else {})},
+                                 "on the SM side (profiles/r1j_cfg3.md)"} if fused23 else {})},
         "path_roofline": {"what": "spread + deconvolve + assembly path = all own kernels except the FFT (total - fft), "
                                   "bytes = streaming model of " + STAGE_BYTES_DOC + "; bytes_sparse = the same with the "
                                   "grid term reduced to the tiles that hold points (what the own-FFT path really writes)",
