@@ -400,12 +400,14 @@ ls_fft_rows_kernel(const FftArgs a) {
 // deadlock.  What a slab's pass 2 writes is read back by its pass 3 a few microseconds later out of the 126 MB L2
 // (ncu: 0.02 % of pass 3's input comes from DRAM), and once read the lines are dead: `discard.global.L2` drops them
 // before they are ever written back.  DRAM traffic of the two passes: 3.0 GB -> 1.48 GB at config 3
-// (profiles/r1g_fft_l2_fusion.md).  lag = 2: one slab is less than half a wave of the 592 resident CTAs.
+// (profiles/r1g_fft_l2_fusion.md).  lag = 3 (measured: lag 1 0.59 ms, 2 0.3965, 3 0.393, 4 0.395, 6 0.435 — one slab
+// is less than half a wave of the 592 resident CTAs, so a short lag makes pass-3 tiles wait and a long one pushes
+// slabs out of L2).
 // After the kernel the fine grids hold indeterminate values; nothing reads them again (the next execute's spreading
 // kernel rewrites every tile that pass 1 will load).
 // queue: [0] next item, [1] CTAs that left, [2 + s] pass-2 tiles of slab s done.  The last CTA to leave zeroes it.
 constexpr int kC23 = 8;                  // tile width of the fused kernel
-constexpr int kLag23 = 2;
+constexpr int kLag23 = 3;
 __device__ __forceinline__ int ld_acquire_gpu(const int* p) {
     int v;
     asm volatile("ld.acquire.gpu.global.s32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
