@@ -342,6 +342,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
                               o.tile_cells > lsb::kSpreadThreads * 4))
         return LS_ERR_INVALID_VALUE;
     if (o.t_is_dtype < 0 || o.t_is_dtype > 1) return LS_ERR_INVALID_VALUE;
+    if (o.reserved[0] < 0 || o.reserved[0] > 2 || o.reserved[1] < 0 || o.reserved[1] > 8) return LS_ERR_INVALID_VALUE;
     if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 3 ||
         o.no_floating_mean < 0 || o.no_floating_mean > 1 || o.normalization < 0 || o.normalization > 3)
         return LS_ERR_INVALID_VALUE;
@@ -749,6 +750,7 @@ int ls_set_workspace(ls_plan_t p, void* dptr, size_t bytes) {
     p->fft_work = base + up(p->grids_bytes) + up(p->modes_bytes);
     p->external_ws = true;
     if (p->gexec) { cudaGraphExecDestroy(p->gexec); p->gexec = nullptr; }     // captured pointers are stale
+    if (p->own_fft && lsb::own_fft_make_tmap(p) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
     if (!p->own_fft) {
         if (cufftSetWorkArea(p->fft_first, p->fft_work) != CUFFT_SUCCESS) return LS_ERR_CUFFT;
         if (p->has_chunk && cufftSetWorkArea(p->fft_chunk, p->fft_work) != CUFFT_SUCCESS) return LS_ERR_CUFFT;

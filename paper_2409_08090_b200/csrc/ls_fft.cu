@@ -21,6 +21,8 @@
 // 16-point FFTs in registers (radix 4 x 4), one shared-memory exchange (conflict-free layouts),
 // 256-byte global segments on both sides.  Twiddles: w_256 from a shared table, w_n^e from two
 // 4096-entry tables (e = 4096 e_hi + e_lo) and a base/step recurrence along the thread's 16 outputs.
+#include <cuda.h>            // CUtensorMap (types only: the encoder is fetched through the runtime, no libcuda link)
+
 #include "ls_internal.h"
 #include "ls_power.cuh"
 
@@ -564,6 +566,285 @@ ls_fft_pass23_kernel(const FftArgs a, int nslabs, int* __restrict__ queue) {
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------------
+// Passes 2 + 3, bulk-asynchronous version (the default for n >= 2^20): the same ordered tile queue, slab signals, L2
+// residency and discard as ls_fft_pass23_kernel above, but the tiles are MOVED by the TMA unit instead of by the
+// threads that compute on them.  One persistent CTA per SM = one producer warp + k23Groups consumer groups of 128
+// threads, a ring of k23Stages shared-memory tile buffers, one full / empty mbarrier pair per buffer:
+//   producer (one elected thread): draws the next queue item, waits for the buffer to be free, waits (pass-3 tiles) for
+//     the slab's pass-2 signal, then issues the tile load — pass-2 tile (256 rows x 128 bytes, rows 4 KB apart): ONE
+//     cp.async.bulk.tensor.3d through a tensor map over [k1][l2][l3]; pass-3 tile (8 rows of 4 KB, 1 MB apart): eight
+//     cp.async.bulk copies into rows padded by one cell (conflict-free second stage) — with complete_tx on the buffer's
+//     full barrier, and prefetches the pass-2 tile one slab ahead into L2 (cp.async.bulk.prefetch.tensor);
+//   consumers: wait on the full barrier, run the first 16-point stage out of shared memory IN PLACE (a thread writes
+//     back exactly the 16 cells it read), one named barrier of their own 128 threads, second stage out of shared memory,
+//     release the buffer (mbarrier arrive) as soon as their operands are in registers, twiddle and store.
+// The 16 data registers x 2 of a thread are therefore never parked on a global load: the loads of the next k23Stages -
+// k23Groups tiles are in flight while every consumer warp computes.
+constexpr int k23Stages = 6;                          // tile buffers in the ring
+constexpr int kLagTma = 3;                            // slabs between a slab's pass 2 and its pass 3 in the queue
+constexpr int k23Batch = 4;                           // consecutive queue items per draw
+__host__ __device__ constexpr int k23threads(int groups) { return (groups * 4 + 1) * 32; }   // consumer groups of 128 threads + the producer warp
+constexpr int k23RowBytes = 4096 + 16;                // a pass-3 tile row (256 cells) padded by one cell
+constexpr int k23BufBytes = 8 * k23RowBytes;          // 32896 >= 32768 (pass-2 tile, dense); a multiple of 128
+constexpr size_t k23TmaSmem = (size_t)k23Stages * k23BufBytes + sizeof(double2) * 3 * 256 + 16 * k23Stages + 4 * k23Stages + 64;
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(unsigned bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    unsigned ok;
+    do {                                                     // try_wait suspends the thread in hardware for a while
+        asm volatile(
+            "{\n\t"
+            ".reg .pred p;\n\t"
+            "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+            "selp.u32 %0, 1, 0, p;\n\t"
+            "}"
+            : "=r"(ok)
+            : "r"(bar), "r"(parity)
+            : "memory");
+    } while (!ok);
+}
+__device__ __forceinline__ void tma_load_3d(unsigned dst, const CUtensorMap* map, unsigned bar, int c0, int c1, int c2) {
+    asm volatile(
+        "cp.async.bulk.tensor.3d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(dst),
+        "l"(map), "r"(bar), "r"(c0), "r"(c1), "r"(c2)
+        : "memory");
+}
+__device__ __forceinline__ void tma_prefetch_3d(const CUtensorMap* map, int c0, int c1, int c2) {
+    asm volatile("cp.async.bulk.prefetch.tensor.3d.L2.global.tile [%0, {%1, %2, %3}];" ::"l"(map), "r"(c0), "r"(c1), "r"(c2)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src),
+                 "r"(bytes), "r"(bar)
+                 : "memory");
+}
+__device__ __forceinline__ void group_barrier(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
+
+template <int k23Groups>                                 // consumer groups (128 threads, one tile at a time each)
+__global__ void __launch_bounds__(k23threads(k23Groups), 1)
+ls_fft_pass23_tma_kernel(const FftArgs a, const __grid_constant__ CUtensorMap tmap, int row0, int nslabs, int lag,
+                         int* __restrict__ queue) {
+    constexpr int C = 8, CT = 256 / C, k23Threads = k23threads(k23Groups);
+    extern __shared__ __align__(128) unsigned char tsm[];
+    unsigned char* bufs = tsm;
+    double2* w256 = reinterpret_cast<double2*>(tsm + (size_t)k23Stages * k23BufBytes);
+    // inter-pass twiddles of pass 2, w_n^{R1 k2 l3} = w_65536^x with x = k2 l3 < 65536, from two 256-entry tables in
+    // shared memory: w_65536^x = wcoarse[x >> 8] wfine[x & 255].  (The 2 x 64 KB global tables of twiddle_n do not fit
+    // the 20 KB of L1 this kernel leaves: their misses sat in front of every tile's stores.)
+    double2* wcoarse = w256 + 256;
+    double2* wfine = wcoarse + 256;
+    unsigned long long* bars = reinterpret_cast<unsigned long long*>(wfine + 256);   // full[k23Stages], empty[k23Stages]
+    int* sitem = reinterpret_cast<int*>(bars + 2 * k23Stages);
+    const unsigned full0 = smem_u32(bars), empty0 = smem_u32(bars + k23Stages);
+    const int warp = threadIdx.x >> 5;
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < k23Stages; ++b) {
+            mbar_init(full0 + 8 * b, 1);               // the producer's arrive.expect_tx (+ the bytes of the tile)
+            mbar_init(empty0 + 8 * b, 128);            // every thread of the consumer group
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    fill_w256(w256, k23Threads);
+    for (int i = threadIdx.x; i < 256; i += k23Threads) {
+        double sn, cs;
+        sincospi((double)i / 128.0, &sn, &cs);
+        wcoarse[i] = make_double2(cs, sn);
+        sincospi((double)i / 32768.0, &sn, &cs);
+        wfine[i] = make_double2(cs, sn);
+    }
+    __syncthreads();
+    const int groups = a.R1 / C;                             // slabs per transform
+    const int total = (nslabs + lag) * 512;
+
+    if (warp == k23Groups * 4) {
+        // ------------------------------------------------------------------------------------------ producer
+        if ((threadIdx.x & 31) == 0) {
+            int filled = 0, terminators = 0;
+            int ready_slabs = 0;                             // slabs [0, ready_slabs) are known to be complete
+            // Items are drawn from the shared counter k23Batch at a time, the next draw always in flight.  One address takes
+            // an atomic with return every ~16 cycles chip-wide (measured: 49 152 single-item draws took 0.39 - 0.44 ms,
+            // whatever the kernel did otherwise — the first version of this kernel AND the per-thread-load kernel above were
+            // both bound by their own work counter), so the draws must be few.
+            int cur = atomicAdd(&queue[0], k23Batch), nxt = atomicAdd(&queue[0], k23Batch), sub = 0;
+            while (terminators < k23Groups) {
+                int item = total;
+                if (terminators == 0) {
+                    item = cur + sub;
+                    if (++sub == k23Batch) {
+                        sub = 0;
+                        cur = nxt;
+                        nxt = cur < total ? atomicAdd(&queue[0], k23Batch) : total;
+                    }
+                }
+                const int buf = filled % k23Stages;
+                const unsigned fb = full0 + 8 * buf, eb = empty0 + 8 * buf;
+                const unsigned dst = smem_u32(bufs + (size_t)buf * k23BufBytes);
+                if (item >= total) {                         // one terminator per consumer group (consecutive ring slots)
+                    mbar_wait(eb, ((filled / k23Stages) & 1) ^ 1);
+                    sitem[buf] = -1;
+                    mbar_arrive(fb);
+                    ++terminators;
+                    ++filled;
+                    continue;
+                }
+                const int b = item >> 9, slot = item & 255;
+                if ((item & 256) == 0) {
+                    // ---- pass-2 tile: row k1 = C g + slot / CT of transform tr, columns C (slot % CT) ..
+                    {
+                        const int it = item + kPrefetch23;   // the same tile of the next slab: HBM -> L2 ahead of its load
+                        const int pb = it >> 9, ps = it & 255;
+                        if (pb < nslabs) {
+                            const int ptr = pb / groups, pg = pb - ptr * groups;
+                            tma_prefetch_3d(&tmap, 2 * C * (ps % CT), 0, row0 + ptr * a.R1 + C * pg + ps / CT);
+                        }
+                    }
+                    if (b >= nslabs) continue;
+                    const int tr = b / groups, g = b - tr * groups;
+                    mbar_wait(eb, ((filled / k23Stages) & 1) ^ 1);
+                    sitem[buf] = item;
+                    mbar_expect_tx(fb, 256 * C * 16);
+                    tma_load_3d(dst, &tmap, fb, 2 * C * (slot % CT), 0, row0 + tr * a.R1 + C * g + slot / CT);
+                } else {
+                    // ---- pass-3 tile: k2 = slot, rows k1 = C g .. C g + C - 1 of the slab drawn `lag` slabs ago
+                    const int sl = b - lag;
+                    if (sl < 0) continue;
+                    const int tr = sl / groups, g = sl - tr * groups;
+                    mbar_wait(eb, ((filled / k23Stages) & 1) ^ 1);
+                    if (sl >= ready_slabs) {                 // slabs complete in queue order (nearly): ask once per slab
+                        const int* done = queue + 2 + sl;
+                        while (ld_acquire_gpu(done) < 256) __nanosleep(40);
+                        asm volatile("fence.proxy.async.global;" ::: "memory");   // the slab was written through the generic proxy
+                        ready_slabs = sl + 1;
+                    }
+                    sitem[buf] = item;
+                    mbar_expect_tx(fb, 256 * C * 16);
+                    const double2* src = a.grids + (long long)tr * a.n + ((long long)(C * g) * 256 + slot) * 256;
+#pragma unroll
+                    for (int c = 0; c < C; ++c) bulk_load(dst + c * k23RowBytes, src + (long long)c * 65536, 4096, fb);
+                }
+                ++filled;
+            }
+        }
+    } else {
+        // ------------------------------------------------------------------------------------------ consumers
+        const int grp = warp >> 2, t = threadIdx.x & 127;
+        // w_256^{16 j} = e^{2 pi i j / 16} for this thread's j in a pass-2 tile (j = t / C) and in a pass-3 tile (j = t % 16)
+        double2 c16_p2, c16_p3;
+        sincospi((double)(t / C) / 8.0, &c16_p2.y, &c16_p2.x);
+        sincospi((double)(t & 15) / 8.0, &c16_p3.y, &c16_p3.x);
+        for (int seq = grp;; seq += k23Groups) {
+            const int buf = seq % k23Stages;
+            mbar_wait(full0 + 8 * buf, (seq / k23Stages) & 1);
+            const int item = sitem[buf];
+            if (item < 0) break;
+            unsigned char* tile = bufs + (size_t)buf * k23BufBytes;
+            const int b = item >> 9, slot = item & 255;
+            double2 x[16];
+            if ((item & 256) == 0) {
+                // ---- pass 2: transform over l2 (the 256 rows of the tile), C columns
+                const int tr = b / groups, g = b - tr * groups;
+                const int k1 = C * g + slot / CT;
+                const int c = t % C, hi4 = t / C;
+                const long long m = (long long)(slot % CT) * C + c;
+                double2* T = reinterpret_cast<double2*>(tile);
+                {
+                    const int j = hi4;
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) x[i] = T[(16 * i + j) * C + c];
+                    fft16(x);
+#pragma unroll
+                    for (int ka = 0; ka <= 8; ++ka) {
+                        if (ka == 0) { T[j * C + c] = x[0]; continue; }
+                        const double2 tw = w256[ka * 16 + j];
+                        T[(ka * 16 + j) * C + c] = cmul(x[pos16(ka)], tw);
+                        if (ka < 8) T[((16 - ka) * 16 + j) * C + c] = cmul(cmul(x[pos16(16 - ka)], c16_p2), make_double2(tw.x, -tw.y));
+                    }
+                }
+                group_barrier(1 + grp);
+                {
+                    const int ka = hi4;
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) x[j] = T[(ka * 16 + j) * C + c];
+                    mbar_arrive(empty0 + 8 * buf);           // operands are in registers: the buffer can be refilled
+                    const unsigned x0 = (unsigned)ka * (unsigned)m, x1 = 16u * (unsigned)m;      // k2 = ka + 16 kb
+                    const double2 tw = cmul(wcoarse[x0 >> 8], wfine[x0 & 255u]);
+                    const double2 st = cmul(wcoarse[x1 >> 8], wfine[x1 & 255u]);
+                    fft16(x);
+                    double2* base = a.grids + (long long)tr * a.n + (long long)k1 * 65536 + m;
+                    store_twiddled<16>(base, 256, ka, tw, st, [&](int kb) { return x[pos16(kb)]; });
+                }
+                group_barrier(1 + grp);                      // every thread's stores are issued ...
+                if (t == 0) {
+                    // ... and ordered before the signal, device-wide, for the generic and the async proxy
+                    asm volatile("fence.proxy.async.global;" ::: "memory");
+                    asm volatile("red.release.gpu.global.add.s32 [%0], 1;" ::"l"(queue + 2 + b) : "memory");
+                }
+            } else {
+                // ---- pass 3: transform over l3 (contiguous), C rows k1 = C g .. at k2 = slot
+                const int sl = b - lag;
+                const int tr = sl / groups, g = sl - tr * groups;
+                const int rho_b = slot * a.R1 + C * g;
+                {
+                    const int j = t & 15, c = t >> 4;
+                    double2* row = reinterpret_cast<double2*>(tile + c * k23RowBytes);
+#pragma unroll
+                    for (int i = 0; i < 16; ++i) x[i] = row[16 * i + j];
+                    {
+                        // the slab is dead once it sits in shared memory: drop its dirty lines from L2 instead of writing
+                        // them back to HBM (thread (c, j) drops lines 2 j and 2 j + 1 of row c's 4 KB chunk)
+                        const double2* grow = a.grids + (long long)tr * a.n + ((long long)(C * g + c) * 256 + slot) * 256 + 16 * j;
+                        asm volatile("discard.global.L2 [%0], 128;" ::"l"(grow) : "memory");
+                        asm volatile("discard.global.L2 [%0], 128;" ::"l"(grow + 8) : "memory");
+                    }
+                    fft16(x);
+#pragma unroll
+                    for (int ka = 0; ka <= 8; ++ka) {
+                        if (ka == 0) { row[j] = x[0]; continue; }
+                        const double2 tw = w256[ka * 16 + j];
+                        row[ka * 16 + j] = cmul(x[pos16(ka)], tw);
+                        if (ka < 8) row[(16 - ka) * 16 + j] = cmul(cmul(x[pos16(16 - ka)], c16_p3), make_double2(tw.x, -tw.y));
+                    }
+                }
+                group_barrier(1 + grp);
+                {
+                    const int c = t % C, ka = t / C;
+                    const double2* row = reinterpret_cast<const double2*>(tile + c * k23RowBytes);
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) x[j] = row[ka * 16 + j];
+                    mbar_arrive(empty0 + 8 * buf);
+                    fft16(x);
+                    double2* out = a.modes + (long long)tr * a.Nf;
+                    const long long kk0 = rho_b + c;
+                    const long long r12 = (long long)a.R1 * 256;
+#pragma unroll
+                    for (int kb = 0; kb < 16; ++kb) {
+                        long long k = kk0 + r12 * (ka + 16 * kb) + a.half;
+                        if (k >= a.n) k -= a.n;
+                        if (k < a.Nf) __stcs(&out[k], x[pos16(kb)]);     // read once, by the assembly, after 600 MB more
+                    }
+                }
+            }
+        }
+    }
+    __syncthreads();                                         // every signal of this CTA has been posted
+    if (threadIdx.x == 0) {
+        if (atomicAdd(&queue[1], 1) == (int)gridDim.x - 1) {  // last CTA out: nobody draws or waits any more
+            for (int i = 0; i < nslabs + 2; ++i) queue[i] = 0;
+        }
+    }
+}
+
 __global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < 4096) {
@@ -612,6 +893,9 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<kC23>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23Smem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass23_tma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23TmaSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_pass23_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23TmaSmem)) != cudaSuccess) return e;
+    if ((e = own_fft_make_tmap(p)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
@@ -683,14 +967,50 @@ cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream
     return cudaGetLastError();
 }
 
+// Tensor map over the plan's fine grids viewed as [rows k1 of every slot][l2 = 256][l3 = 256 cells = 512 doubles]
+// (n >= 2^20: a pass-1 output row k1 is 65536 cells = 1 MB), box = one pass-2 tile: 8 cells x 256 rows l2 of one k1.
+// The encoder is a driver entry point fetched through the runtime (no link against libcuda).  Called at plan time and
+// whenever the grids move (ls_set_workspace).
+cudaError_t own_fft_make_tmap(ls_plan_s* p) {
+    if (!p->fuse_pass23) return cudaSuccess;
+    static_assert(sizeof(CUtensorMap) <= sizeof(p->fft_tmap), "tensor map storage");
+    void* fn = nullptr;
+    cudaDriverEntryPointQueryResult qres;
+    cudaError_t e = cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres);
+    if (e != cudaSuccess) return e;
+    if (qres != cudaDriverEntryPointSuccess || !fn) return cudaErrorNotSupported;
+    typedef CUresult (*encode_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                 const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                 CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    const cuuint64_t rows = (cuuint64_t)p->slots * (cuuint64_t)(p->n / 65536);
+    const cuuint64_t dims[3] = {512, 256, rows};
+    const cuuint64_t strides[2] = {4096, 1048576};           // bytes: l2 -> l2 + 1, k1 -> k1 + 1
+    const cuuint32_t box[3] = {2 * kC23, 256, 1}, estr[3] = {1, 1, 1};
+    const CUresult r = ((encode_t)fn)(reinterpret_cast<CUtensorMap*>(p->fft_tmap), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, 3, p->grids,
+                                      dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                      CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    return r == CUDA_SUCCESS ? cudaSuccess : cudaErrorInvalidValue;
+}
+
 // Passes 2 and 3 of transforms [slot0, slot0 + ntrans) in one persistent kernel (n >= 2^20): compact modes out,
-// fine grids left indeterminate.
+// fine grids left indeterminate.  Default: the bulk-asynchronous (TMA + mbarrier) kernel, one CTA per SM;
+// opts.reserved[0] = 1 selects the first version (per-thread loads, four 128-thread CTAs per SM), kept for comparison.
 cudaError_t launch_own_fft_pass23(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
     FftArgs a;
     fill_common(p, a, slot0, 0);
     const int nslabs = ntrans * (a.R1 / kC23);
-    const int nblk = std::min(nslabs * 256, (512 / (16 * kC23)) * p->num_sms);
-    ls_fft_pass23_kernel<kC23><<<nblk, 16 * kC23, k23Smem, s>>>(a, nslabs, p->fft_queue);
+    if (p->opts.reserved[0] == 1) {
+        const int nblk = std::min(nslabs * 256, (512 / (16 * kC23)) * p->num_sms);
+        ls_fft_pass23_kernel<kC23><<<nblk, 16 * kC23, k23Smem, s>>>(a, nslabs, p->fft_queue);
+        return cudaGetLastError();
+    }
+    const int nblk = std::min(nslabs * 256, p->num_sms);
+    const CUtensorMap& tm = *reinterpret_cast<const CUtensorMap*>(p->fft_tmap);
+    const int lag = p->opts.reserved[1] ? p->opts.reserved[1] : kLagTma;
+    if (p->opts.reserved[0] == 2)
+        ls_fft_pass23_tma_kernel<3><<<nblk, k23threads(3), k23TmaSmem, s>>>(a, tm, slot0 * a.R1, nslabs, lag, p->fft_queue);
+    else
+        ls_fft_pass23_tma_kernel<4><<<nblk, k23threads(4), k23TmaSmem, s>>>(a, tm, slot0 * a.R1, nslabs, lag, p->fft_queue);
     return cudaGetLastError();
 }
 

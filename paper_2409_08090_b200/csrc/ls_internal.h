@@ -120,6 +120,7 @@ struct ls_plan_s {
     int* tile_counts = nullptr;                     // [2] list lengths (in `zeroed`)
     int* fft_queue = nullptr;                       // [2 + 16 slots] work queue of the fused FFT passes 2 + 3 (in `zeroed`)
     unsigned* row_masks = nullptr;                  // [2][65536/L][<=16] liveness bits for FFT pass 1 (in `zeroed`)
+    alignas(64) unsigned char fft_tmap[128] = {0};  // CUtensorMap over the fine grids (pass-2 tiles of the fused FFT kernel)
     // CUDA-graph replay of the execute sequence (launch-latency-bound small problems; opts.graph)
     bool use_graph = false;
     cudaGraphExec_t gexec = nullptr;
@@ -154,6 +155,7 @@ bool own_fft_supported(const ls_plan_s* p);
 bool own_fft_prunes(const ls_plan_s* p);          // first pass pruned by liveness masks (n >= 2^20)
 int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 (where that pass is the 16 x RB kernel)
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
+cudaError_t own_fft_make_tmap(ls_plan_s* p);      // (re-)encode the tensor map of the fine grids (plan, ls_set_workspace)
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s);
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
 cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
