@@ -58,6 +58,7 @@ def parse_args():
     ap.add_argument("--fft-impl", type=int, default=0, help="0 auto, 1 cuFFT, 2 own FFT with the last pass fused into the assembly, 3 own FFT unfused")
     ap.add_argument("--graph", type=int, default=0, help="0 auto, 1 never, 2 always (user-facing plan)")
     ap.add_argument("--variant", type=int, default=0, help="ls_opts.reserved[0]: kernel variant kept for comparison")
+    ap.add_argument("--lag", type=int, default=0, help="ls_opts.reserved[1]: queue lag of the fused FFT kernels (0 = default)")
     return ap.parse_args()
 
 
@@ -296,8 +297,8 @@ def run_ours(args):
     flush = torch.empty(512 << 20, dtype=torch.uint8, device=dev)
     popts = dict(device=local, tile_cells=args.tile_cells, upsampfac=args.upsampfac,
                  kernel_width=args.kernel_width, batch_chunk=args.batch_chunk, fft_impl=args.fft_impl)
-    if args.variant:
-        popts["reserved"] = (args.variant, 0)
+    if args.variant or args.lag:
+        popts["reserved"] = (args.variant, args.lag)
     ldt = B.LS_F64 if w.dtype == "f64" else B.LS_F32
     # Two plans: `plan` is what a user runs (no stage events; small problems replay a CUDA graph; with the own FFT
     # the last pass is fused with the assembly) and gives `value`; `plan_t` records CUDA events around every

@@ -86,11 +86,18 @@ enum {
 /* Optional tuning; a zero-initialised struct (or NULL) selects the defaults. */
 typedef struct {
     int dy_per_series;      /* 0: dy[Nd] shared by the batch (A13, default); 1: dy[batch][Nd]     */
-    double upsampfac;       /* sigma; 0 = auto (2.0)                                              */
-    int kernel_width;       /* w in fine-grid cells; 0 = auto from eps (A10)                      */
+    double upsampfac;       /* sigma; 0 = auto: n = the power of two in [1.25 Nf, 2.5 Nf) (or, where that is much
+                               larger than needed, the fastest of a few timed smooth sizes: the choice is cached
+                               per process, and may differ between processes / devices, as do the last bits of the
+                               results: scatter order inside a sort bin and the statistics' atomic sums are
+                               unordered).  Non-zero: n = the smallest even 5-smooth size >= upsampfac * Nf   */
+    int kernel_width;       /* w in fine-grid cells, 2..20; 0 = auto from eps (A10).  The kernels hold at most 20
+                               cells: where eps needs more at the automatic sigma the grid doubles; with a fixed
+                               upsampfac the plan is refused with LS_ERR_UNSUPPORTED                        */
     int timing;             /* 1: record CUDA events around each stage of every execute           */
     int device;             /* CUDA device ordinal the plan lives on                              */
-    int tile_cells;         /* spreading tile length L in cells; 0 = auto                         */
+    int tile_cells;         /* spreading tile length L in cells: 256, 512 or 1024 (1024: single series only);
+                               0 = auto                                                           */
     int batch_chunk;        /* series spread/FFT'd/assembled per pass; 0 = auto (<= 8 GB of grids)  */
     int no_autotune;        /* 1: never time candidate grid sizes at plan time (auto n = power of two) */
     int graph;              /* CUDA-graph replay of the execute sequence (needs timing == 0 and a non-legacy
@@ -117,9 +124,11 @@ typedef struct {
  * carefully chosen to match the user tolerance"; A10), build the deconvolution table
  * 1/psihat(k') ("diagonal rescaling"), the cuFFT plan and all scratch buffers.
  *   Nd >= 1 points, Nf >= 1 frequencies, f0 >= 0 and df > 0 finite (cycles per unit of t),
- *   eps in [1e-14, 1e-1] for LS_F64 / [1e-6, 1e-1] for LS_F32, batch >= 1.
+ *   eps in [1e-14, 1e-1] for LS_F64 / [1e-6, 1e-1] for LS_F32, 1 <= batch <= 65535 (a grid dimension
+ *   of the per-series kernels).
  * Errors: LS_ERR_INVALID_VALUE for anything outside those ranges or out == NULL;
- * LS_ERR_UNSUPPORTED if the fine grid needs n >= 2^31 cells; LS_ERR_ALLOC / _CUDA / _CUFFT. */
+ * LS_ERR_UNSUPPORTED if the fine grid needs n >= 2^31 cells, or a fixed upsampfac needs a kernel wider than 20
+ * cells for eps; LS_ERR_ALLOC / _CUDA / _CUFFT. */
 int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double eps,
             int dtype, int batch, const ls_opts* opts /* NULL ok */);
 
@@ -174,6 +183,24 @@ int ls_get_launch_counts(ls_plan_t plan, int* own_kernels, int* fft_execs);
 int ls_debug_modes(ls_plan_t plan, int series, int64_t K, const int64_t* kidx, double* out);
 int ls_debug_stats(ls_plan_t plan, double* out);
 
+/* Stage pins (SURVEY.md §8(c) "Stage pins for GPU kernels"): intermediates of single stages, all HOST output buffers,
+ * all synchronise the device.  Layouts are those of the kernels and may change with them.
+ *   ls_debug_points: the bin-sorted point records of the most recent execute, point set 0 (x1 = n df t) or 1
+ *     (x2 = 2 x1): out[Nd][4] = (eta, l0, q_re, q_im); l0 = first fine-grid cell the point touches (unfolded),
+ *     eta = 2 (l0 - u) + (w - 1) in [-1, 1) with u the point's grid coordinate; q = w_j e^{2 pi i f_c t_j} (x1) or
+ *     w_j e^{4 pi i f_c t_j} (x2) when dy is shared by the batch, the unit phasor otherwise.
+ *   ls_debug_bins: out[nbins + 1] = first sorted slot of every sort bin of 64 cells (nbins = ceil(n / 64)).
+ *   ls_debug_grid: runs K1..K4 on (t, y, dy) (device pointers, legacy stream) and returns fine grid `slot` as the
+ *     spreading kernel left it: out[n][2].  LS_ERR_UNSUPPORTED where empty tiles are not written (own FFT, n >= 2^20).
+ *   ls_debug_dinv: out[i] = 1 / psihat(k') at |k'| = kabs[i] <= Nf / 2 (the P0 table).
+ *   ls_debug_assemble: K6 alone (no plan): power of K frequencies from sums[K][6] = (Sh, Ch, S, C, S2, C2). */
+int ls_debug_points(ls_plan_t plan, int set, double* out);
+int ls_debug_bins(ls_plan_t plan, int set, int* out);
+int ls_debug_grid(ls_plan_t plan, const void* t, const void* y, const void* dy, int slot, double* out);
+int ls_debug_dinv(ls_plan_t plan, int64_t K, const int64_t* kabs, double* out);
+int ls_debug_assemble(int64_t K, const double* sums, double YY, double W, int no_floating_mean, int normalization,
+                      double* out);
+
 /* ls_direct_power — verification path, NOT part of ls_execute: the six sums of
  * Eq. 1 evaluated by brute force, O(Nd K), for the K consecutive frequencies
  * f0 + (k0 + i) df, i = 0..K-1, of ONE fp64 series, then the same power assembly.  The kind of direct
@@ -184,6 +211,14 @@ int ls_debug_stats(ls_plan_t plan, double* out);
  * Errors: LS_ERR_INVALID_VALUE, LS_ERR_ALLOC, LS_ERR_CUDA. */
 int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
                     const void* dy, void* power, void* cuda_stream);
+
+/* ls_direct_sums — the same brute-force evaluation, but returning the six sums themselves and NOT the power:
+ *   sums  device, double[K][6] = (Sh, Ch, S, C, S2, C2) of frequency f0 + (k0 + i) df (written).
+ * None of the library's assembly arithmetic (tau, CC, SS) is involved, so a test can put these sums through the
+ * ORACLE's assembly and check the NUFFT path's K6 independently of ls_power.cuh.  Same scratch, stream and error
+ * behaviour as ls_direct_power. */
+int ls_direct_sums(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                   const void* dy, void* sums, void* cuda_stream);
 
 const char* ls_strerror(int code);
 

@@ -14,7 +14,8 @@ import os
 __all__ = [
     "LS_F32", "LS_F64", "LS_OK", "STAGES", "LsError", "ls_opts", "lib_path", "load",
     "ls_plan", "ls_execute", "ls_execute_host", "ls_destroy", "ls_get_info", "ls_workspace_bytes", "ls_set_workspace",
-    "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_strerror", "ls_direct_power",
+    "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_debug_points", "ls_debug_bins", "ls_debug_grid", "ls_debug_dinv",
+    "ls_debug_assemble", "ls_strerror", "ls_direct_power", "ls_direct_sums",
     "exported_symbols", "Plan",
 ]
 
@@ -68,7 +69,14 @@ _SIGNATURES = {
     "ls_get_launch_counts": (C.c_int, [C.c_void_p, C.POINTER(C.c_int), C.POINTER(C.c_int)]),
     "ls_debug_modes": (C.c_int, [C.c_void_p, C.c_int, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]),
     "ls_debug_stats": (C.c_int, [C.c_void_p, C.POINTER(C.c_double)]),
+    "ls_debug_points": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
+    "ls_debug_bins": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int)]),
+    "ls_debug_grid": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
+    "ls_debug_dinv": (C.c_int, [C.c_void_p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]),
+    "ls_debug_assemble": (C.c_int, [C.c_int64, C.POINTER(C.c_double), C.c_double, C.c_double, C.c_int, C.c_int,
+                                    C.POINTER(C.c_double)]),
     "ls_direct_power": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
+    "ls_direct_sums": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
     "ls_strerror": (C.c_char_p, [C.c_int]),
     "ls_destroy": (C.c_int, [C.c_void_p]),
 }
@@ -171,6 +179,14 @@ def ls_direct_power(Nd, f0, df, k0, K, t, y, dy, power, stream=0) -> None:
         raise LsError(rc, "ls_direct_power")
 
 
+def ls_direct_sums(Nd, f0, df, k0, K, t, y, dy, sums, stream=0) -> None:
+    """The six brute-force sums (Sh, Ch, S, C, S2, C2) of frequencies f0 + (k0 .. k0+K-1) df into sums[K][6] (device)."""
+    rc = load().ls_direct_sums(int(Nd), float(f0), float(df), int(k0), int(K), C.c_void_p(_ptr(t)), C.c_void_p(_ptr(y)),
+                               C.c_void_p(_ptr(dy)), C.c_void_p(_ptr(sums)), C.c_void_p(int(stream)))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_direct_sums")
+
+
 def ls_get_stage_ms(plan) -> dict:
     ms = (C.c_float * len(STAGES))()
     rc = load().ls_get_stage_ms(plan, ms, len(STAGES))
@@ -204,6 +220,59 @@ def ls_debug_stats(plan, batch):
     rc = load().ls_debug_stats(plan, out.ctypes.data_as(C.POINTER(C.c_double)))
     if rc != LS_OK:
         raise LsError(rc, "ls_debug_stats")
+    return out
+
+
+def _dp(a):
+    return a.ctypes.data_as(C.POINTER(C.c_double))
+
+
+def ls_debug_points(plan, Nd, point_set):
+    """Bin-sorted point records of the last execute: [Nd, 4] = (eta, l0, q_re, q_im); point_set 0 = x1, 1 = x2."""
+    import numpy as np
+    out = np.empty((int(Nd), 4), dtype=np.float64)
+    rc = load().ls_debug_points(plan, int(point_set), _dp(out))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_debug_points")
+    return out
+
+
+def ls_debug_bins(plan, nbins, point_set):
+    import numpy as np
+    out = np.empty(int(nbins) + 1, dtype=np.int32)
+    rc = load().ls_debug_bins(plan, int(point_set), out.ctypes.data_as(C.POINTER(C.c_int)))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_debug_bins")
+    return out
+
+
+def ls_debug_grid(plan, n, t, y, dy, slot):
+    """Fine grid `slot` ([n] complex128) after K1..K4 on the device buffers t, y, dy."""
+    import numpy as np
+    out = np.empty((int(n), 2), dtype=np.float64)
+    rc = load().ls_debug_grid(plan, C.c_void_p(_ptr(t)), C.c_void_p(_ptr(y)), C.c_void_p(_ptr(dy)), int(slot), _dp(out))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_debug_grid")
+    return out[:, 0] + 1j * out[:, 1]
+
+
+def ls_debug_dinv(plan, kabs):
+    import numpy as np
+    k = np.ascontiguousarray(kabs, dtype=np.int64)
+    out = np.empty(k.size, dtype=np.float64)
+    rc = load().ls_debug_dinv(plan, k.size, k.ctypes.data_as(C.POINTER(C.c_int64)), _dp(out))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_debug_dinv")
+    return out
+
+
+def ls_debug_assemble(sums, YY, W=1.0, no_floating_mean=0, normalization=0):
+    import numpy as np
+    s = np.ascontiguousarray(sums, dtype=np.float64).reshape(-1, 6)
+    out = np.empty(s.shape[0], dtype=np.float64)
+    rc = load().ls_debug_assemble(s.shape[0], _dp(s), float(YY), float(W), int(no_floating_mean), int(normalization), _dp(out))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_debug_assemble")
     return out
 
 

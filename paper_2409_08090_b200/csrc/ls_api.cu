@@ -6,7 +6,10 @@
 #include <string.h>
 
 #include <algorithm>
+#include <map>
+#include <mutex>
 #include <new>
+#include <tuple>
 
 #include "ls_internal.h"
 
@@ -338,9 +341,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     if (opts) o = *opts;
     if (o.upsampfac != 0.0 && !(o.upsampfac >= 1.2 && o.upsampfac <= 4.0)) return LS_ERR_INVALID_VALUE;
     if (o.kernel_width != 0 && (o.kernel_width < 2 || o.kernel_width > lsb::kMaxWidth)) return LS_ERR_INVALID_VALUE;
-    if (o.tile_cells != 0 && (o.tile_cells % lsb::kBinCells != 0 || o.tile_cells < lsb::kBinCells ||
-                              o.tile_cells > lsb::kSpreadThreads * 4))
-        return LS_ERR_INVALID_VALUE;
+    // spreading tiles: one, two or four cells per thread of a 256-thread CTA (the instantiated kernels); a batch
+    // accumulates four transforms per CTA and has registers for two cells per thread
+    if (o.tile_cells != 0 && o.tile_cells != 256 && o.tile_cells != 512 && o.tile_cells != 1024) return LS_ERR_INVALID_VALUE;
+    if (o.tile_cells == 1024 && batch > 1) return LS_ERR_INVALID_VALUE;
     if (o.t_is_dtype < 0 || o.t_is_dtype > 1) return LS_ERR_INVALID_VALUE;
     if (o.reserved[0] < 0 || o.reserved[0] > 2 || o.reserved[1] < 0 || o.reserved[1] > 8) return LS_ERR_INVALID_VALUE;
     if (o.batch_chunk < 0 || o.graph < 0 || o.graph > 2 || o.fft_impl < 0 || o.fft_impl > 3 ||
@@ -375,22 +379,42 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         while ((double)m < want) m *= 2;
         p->n = m;
         const int ntrans = o.dy_per_series ? 3 * batch : batch + 2;
-        if ((double)m > 1.6 * (double)Nf && (double)m * ntrans >= (double)((int64_t)1 << 20) && !o.no_autotune)
-            p->n = autotune_grid_size(Nf, dtype, m, ntrans);
+        if ((double)m > 1.6 * (double)Nf && (double)m * ntrans >= (double)((int64_t)1 << 20) && !o.no_autotune) {
+            // the timed choice is cached per (Nf, dtype, transforms, device): the same arguments give the same grid — and
+            // therefore the same results — for the life of the process (between processes it may differ: ls.h)
+            static std::mutex mu;
+            static std::map<std::tuple<int64_t, int, int, int>, int64_t> cache;
+            std::lock_guard<std::mutex> lock(mu);
+            const auto key = std::make_tuple(Nf, dtype, ntrans, o.device);
+            auto it = cache.find(key);
+            if (it == cache.end()) it = cache.emplace(key, autotune_grid_size(Nf, dtype, m, ntrans)).first;
+            p->n = it->second;
+        }
     }
     if (p->n >= ((int64_t)1 << 31) - 4096) { delete p; return LS_ERR_UNSUPPORTED; }
     p->sigma = (double)p->n / (double)Nf;
     int w = o.kernel_width;
     if (w == 0) {
         const double s = std::min(p->sigma, 2.0);      // tiny Nf: n is floored at 64 cells
-        const double rate = M_PI * sqrt(1.0 - 1.0 / s);
         // Measured (single point, sup norm over its position): the ES kernel's error is
         // ~ 30 exp(-w rate) for sigma in [1.25, 2].  fp64: aim a decade below eps so that a pointwise
         // reading of the tolerance holds too (A8) — 12 cells at sigma = 2, 17 at 1.34, 19 at 1.25, for
         // eps = 1e-9.  fp32: the grid's own rounding (6e-8) dominates early; the plain rule plus one cell.
-        if (dtype == LS_F64) w = (int)ceil((-log(eps) + log(300.0)) / rate - 1e-9);
-        else w = (int)ceil(-log(eps) / rate - 1e-9) + 1;
-        w = std::max(2, std::min(lsb::kMaxWidth, w));
+        auto width_for = [&](double sg) {
+            const double rt = M_PI * sqrt(1.0 - 1.0 / std::min(sg, 2.0));
+            return dtype == LS_F64 ? (int)ceil((-log(eps) + log(300.0)) / rt - 1e-9) : (int)ceil(-log(eps) / rt - 1e-9) + 1;
+        };
+        w = width_for(s);
+        // The kernels hold at most kMaxWidth cells.  Where the tolerance asks for more at this sigma, the automatic grid
+        // doubles (sigma >= 2 needs <= 17 cells down to eps = 1e-14); with a grid size the caller fixed, the plan is refused
+        // rather than silently missing the tolerance.
+        while (w > lsb::kMaxWidth && o.upsampfac == 0.0 && p->n < ((int64_t)1 << 30)) {
+            p->n *= 2;
+            p->sigma = (double)p->n / (double)Nf;
+            w = width_for(p->sigma);
+        }
+        if (w > lsb::kMaxWidth) { delete p; return LS_ERR_UNSUPPORTED; }
+        w = std::max(2, w);
     }
     p->w = w;
     p->beta = 0.97 * M_PI * w * (1.0 - 1.0 / (2.0 * std::min(p->sigma, 2.0)));
@@ -592,6 +616,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 w2_slot = 0; w2_stride = 0; w_slot = 1; w_stride = 0; h_slot = 2; h_stride = 1;
             }
             stage_end(p, s);
+            if (p->debug_stop_after_spread) break;      // ls_debug_grid: the fine grids as the spreading kernel left them
 
             if (p->own_fft) {
                 // own three-pass FFT: pass 1 skips the tiles spreading left unwritten; pass 3 emits compact modes
@@ -822,6 +847,77 @@ int ls_debug_modes(ls_plan_t p, int series, int64_t K, const int64_t* kidx, doub
                         cudaMemcpy(out, dout, K * 48, cudaMemcpyDeviceToHost) != cudaSuccess))
         rc = LS_ERR_CUDA;
     cudaFree(dk);
+    cudaFree(dout);
+    if (rc != LS_OK) cudaGetLastError();
+    return rc;
+}
+
+// ---- stage pins (tests only): intermediates of the pre-processing, spreading and assembly stages ------------------
+int ls_debug_points(ls_plan_t p, int set, double* out) {
+    if (!p || !out || set < 0 || set > 1) return LS_ERR_INVALID_VALUE;
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    const size_t Nd = (size_t)p->Nd;
+    if (p->dtype == LS_F64) {
+        std::vector<lsb::Rec64> h(Nd);
+        if (cudaMemcpy(h.data(), p->ps[set].rec, Nd * sizeof(lsb::Rec64), cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+        for (size_t i = 0; i < Nd; ++i) { out[4 * i] = h[i].eta; out[4 * i + 1] = h[i].l0; out[4 * i + 2] = h[i].qx; out[4 * i + 3] = h[i].qy; }
+    } else {
+        std::vector<lsb::Rec32> h(Nd);
+        if (cudaMemcpy(h.data(), p->ps[set].rec, Nd * sizeof(lsb::Rec32), cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+        for (size_t i = 0; i < Nd; ++i) { out[4 * i] = h[i].eta; out[4 * i + 1] = h[i].l0; out[4 * i + 2] = h[i].qx; out[4 * i + 3] = h[i].qy; }
+    }
+    return LS_OK;
+}
+
+int ls_debug_bins(ls_plan_t p, int set, int* out) {
+    if (!p || !out || set < 0 || set > 1) return LS_ERR_INVALID_VALUE;
+    if (cudaDeviceSynchronize() != cudaSuccess ||
+        cudaMemcpy(out, p->ps[set].bin_start, (size_t)(p->nbins + 1) * 4, cudaMemcpyDeviceToHost) != cudaSuccess) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    return LS_OK;
+}
+
+int ls_debug_grid(ls_plan_t p, const void* t, const void* y, const void* dy, int slot, double* out) {
+    if (!p || !t || !y || !dy || !out || slot < 0 || slot >= p->slots) return LS_ERR_INVALID_VALUE;
+    if (p->fft_prune) return LS_ERR_UNSUPPORTED;           // tiles without points do not exist on the pruned path
+    p->debug_stop_after_spread = true;
+    const int rc = enqueue_execute(p, t, y, dy, nullptr, 0);
+    p->debug_stop_after_spread = false;
+    if (rc != LS_OK) return rc;
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    const size_t n = (size_t)p->n;
+    if (p->dtype == LS_F64) {
+        if (cudaMemcpy(out, (const char*)p->grids + (size_t)slot * n * 16, n * 16, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    } else {
+        std::vector<float> h(2 * n);
+        if (cudaMemcpy(h.data(), (const char*)p->grids + (size_t)slot * n * 8, n * 8, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+        for (size_t i = 0; i < 2 * n; ++i) out[i] = h[i];
+    }
+    return LS_OK;
+}
+
+int ls_debug_dinv(ls_plan_t p, int64_t K, const int64_t* kabs, double* out) {
+    if (!p || !kabs || !out || K < 1) return LS_ERR_INVALID_VALUE;
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    for (int64_t i = 0; i < K; ++i) {
+        if (kabs[i] < 0 || kabs[i] > p->Nf / 2) return LS_ERR_INVALID_VALUE;
+        if (cudaMemcpy(out + i, p->dinv + kabs[i], 8, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    }
+    return LS_OK;
+}
+
+int ls_debug_assemble(int64_t K, const double* sums, double YY, double W, int no_floating_mean, int normalization, double* out) {
+    if (!sums || !out || K < 1 || normalization < 0 || normalization > 3) return LS_ERR_INVALID_VALUE;
+    double *ds = nullptr, *dout = nullptr;
+    int rc = LS_OK;
+    if (cudaMalloc((void**)&ds, K * 48) != cudaSuccess || cudaMalloc((void**)&dout, K * 8) != cudaSuccess) rc = LS_ERR_ALLOC;
+    if (rc == LS_OK && (cudaMemcpy(ds, sums, K * 48, cudaMemcpyHostToDevice) != cudaSuccess ||
+                        lsb::launch_debug_assemble(K, ds, YY, W, no_floating_mean, normalization, dout, 0) != cudaSuccess ||
+                        cudaMemcpy(out, dout, K * 8, cudaMemcpyDeviceToHost) != cudaSuccess))
+        rc = LS_ERR_CUDA;
+    cudaFree(ds);
     cudaFree(dout);
     if (rc != LS_OK) cudaGetLastError();
     return rc;

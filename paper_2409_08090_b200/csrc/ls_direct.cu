@@ -73,7 +73,7 @@ __global__ void ls_direct_prepare_kernel(const double* __restrict__ t, const dou
 
 __global__ void __launch_bounds__(kDirThreads)
 ls_direct_kernel(const DirPoint* __restrict__ pts, long long Nd, double f0, double df, long long k0, long long K,
-                 const double* __restrict__ sums, double* __restrict__ power) {
+                 const double* __restrict__ sums, double* __restrict__ power, double* __restrict__ raw) {
     __shared__ DirPoint sp[kTilePts];
     const long long kfirst = ((long long)blockIdx.x * kDirThreads + threadIdx.x) * kR;   // offset inside [0, K)
     // f = f0 + (k0 + kfirst) df as a double-double (error-free product + two-sum)
@@ -116,6 +116,15 @@ ls_direct_kernel(const DirPoint* __restrict__ pts, long long Nd, double f0, doub
         }
     }
     if (kfirst >= K) return;
+    if (raw != nullptr) {                       // ls_direct_sums: the six sums themselves, no assembly
+#pragma unroll
+        for (int r = 0; r < kR; ++r)
+            if (kfirst + r < K) {
+                double* o = raw + 6 * (kfirst + r);
+                o[0] = Sh[r]; o[1] = Ch[r]; o[2] = S[r]; o[3] = C[r]; o[4] = S2[r]; o[5] = C2[r];
+            }
+        return;
+    }
     const double inv_YY = 1.0 / sums[2];
 #pragma unroll
     for (int r = 0; r < kR; ++r)
@@ -125,10 +134,10 @@ ls_direct_kernel(const DirPoint* __restrict__ pts, long long Nd, double f0, doub
 }  // namespace
 }  // namespace lsb
 
-extern "C" int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
-                               const void* dy, void* power, void* cuda_stream) {
+static int direct_run(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y, const void* dy,
+                      void* power, void* raw, void* cuda_stream) {
     using namespace lsb;
-    if (Nd < 1 || K < 1 || k0 < 0 || !t || !y || !dy || !power || !(df > 0.0) || !(f0 >= 0.0)) return LS_ERR_INVALID_VALUE;
+    if (Nd < 1 || K < 1 || k0 < 0 || !t || !y || !dy || (!power && !raw) || !(df > 0.0) || !(f0 >= 0.0)) return LS_ERR_INVALID_VALUE;
     cudaStream_t s = (cudaStream_t)cuda_stream;
     double* sums = nullptr;
     DirPoint* pts = nullptr;
@@ -145,11 +154,23 @@ extern "C" int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int
         ls_direct_prepare_kernel<<<nb, 256, 0, s>>>((const double*)t, (const double*)y, (const double*)dy, Nd, df, sums, pts);
         const long long threads = (K + kR - 1) / kR;
         ls_direct_kernel<<<(unsigned)((threads + kDirThreads - 1) / kDirThreads), kDirThreads, 0, s>>>(
-            pts, Nd, f0, df, k0, K, sums, (double*)power);
+            pts, Nd, f0, df, k0, K, sums, (double*)power, (double*)raw);
         if (cudaGetLastError() != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) rc = LS_ERR_CUDA;
     }
     cudaFree(sums);
     cudaFree(pts);
     if (rc != LS_OK) cudaGetLastError();
     return rc;
+}
+
+extern "C" int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                               const void* dy, void* power, void* cuda_stream) {
+    if (!power) return LS_ERR_INVALID_VALUE;
+    return direct_run(Nd, f0, df, k0, K, t, y, dy, power, nullptr, cuda_stream);
+}
+
+extern "C" int ls_direct_sums(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                              const void* dy, void* sums, void* cuda_stream) {
+    if (!sums) return LS_ERR_INVALID_VALUE;
+    return direct_run(Nd, f0, df, k0, K, t, y, dy, nullptr, sums, cuda_stream);
 }

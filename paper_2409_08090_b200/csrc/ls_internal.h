@@ -132,6 +132,7 @@ struct ls_plan_s {
     size_t events_used = 0;
     bool timed_once = false;
     int own_kernels = 0, fft_execs = 0;
+    bool debug_stop_after_spread = false;   // ls_debug_grid
     double model_bytes = 0;
 };
 
@@ -168,5 +169,7 @@ cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, 
                             int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s);
 cudaError_t launch_debug_modes(ls_plan_s* p, int h_slot, int w_slot, int w2_slot, int64_t K,
                                const int64_t* d_kidx, double* d_out, cudaStream_t s);
+cudaError_t launch_debug_assemble(int64_t K, const double* d_sums, double YY, double W, int no_float, int norm,
+                                  double* d_out, cudaStream_t s);
 
 }  // namespace lsb

@@ -127,7 +127,23 @@ __global__ void ls_debug_modes_kernel(const void* grids, long long n, long long 
     o[4] = (double)g2.y * d; o[5] = (double)g2.x * d;
 }
 
+// K6 alone, on sums handed in by a test (stage pin: the oracle's exact sums in, power out)
+__global__ void ls_debug_assemble_kernel(long long K, const double* __restrict__ sums, double YY, double W, int no_float,
+                                         int norm, double* __restrict__ out) {
+    const long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= K) return;
+    const double* g = sums + 6 * q;                  // (Sh, Ch, S, C, S2, C2)
+    const double P = assemble_power(g[0], g[1], no_float ? 0.0 : g[2], no_float ? 0.0 : g[3], g[4], g[5], 1.0 / YY);
+    out[q] = apply_normalization(P, norm, YY, W);
+}
+
 }  // namespace
+
+cudaError_t launch_debug_assemble(int64_t K, const double* d_sums, double YY, double W, int no_float, int norm,
+                                  double* d_out, cudaStream_t s) {
+    ls_debug_assemble_kernel<<<(unsigned)((K + 127) / 128), 128, 0, s>>>(K, d_sums, YY, W, no_float, norm, d_out);
+    return cudaGetLastError();
+}
 
 cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double* weights, cudaStream_t s) {
     const long long count = p->Nf / 2 + 1;

@@ -34,23 +34,23 @@ def test_library_builds_and_exports_every_declared_symbol():
 
 
 def test_ls_opts_layout_matches_header():
-    """sizeof/offsets of the ctypes mirror against the C declaration order (int,double,int,int,int,int,int,int[8])."""
+    """Offsets and size of the ctypes mirror against what gcc computes from include/ls.h itself."""
+    import subprocess, tempfile
     from paper_2409_08090_b200.binding import ls_opts
-    assert ls_opts.dy_per_series.offset == 0
-    assert ls_opts.upsampfac.offset == 8
-    assert ls_opts.kernel_width.offset == 16
-    assert ls_opts.timing.offset == 20
-    assert ls_opts.device.offset == 24
-    assert ls_opts.tile_cells.offset == 28
-    assert ls_opts.batch_chunk.offset == 32
-    assert ls_opts.no_autotune.offset == 36
-    assert ls_opts.graph.offset == 40
-    assert ls_opts.fft_impl.offset == 44
-    assert ls_opts.no_floating_mean.offset == 48
-    assert ls_opts.normalization.offset == 52
-    assert ls_opts.t_is_dtype.offset == 56
-    assert ls_opts.reserved.offset == 60
-    assert ctypes.sizeof(ls_opts) == 72
+    names = [f[0] for f in ls_opts._fields_]
+    prog = '#include <stdio.h>\n#include <stddef.h>\n#include "ls.h"\nint main(void){\n'
+    for n in names:
+        prog += f'  printf("{n} %zu\\n", offsetof(ls_opts, {n}));\n'
+    prog += '  printf("sizeof %zu\\n", sizeof(ls_opts));\n  return 0;\n}\n'
+    with tempfile.TemporaryDirectory() as d:
+        src, exe = os.path.join(d, "o.c"), os.path.join(d, "o")
+        with open(src, "w") as f:
+            f.write(prog)
+        subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), src, "-o", exe], check=True)
+        out = dict(l.split() for l in subprocess.run([exe], check=True, capture_output=True, text=True).stdout.splitlines())
+    for n in names:
+        assert getattr(ls_opts, n).offset == int(out[n]), n
+    assert ctypes.sizeof(ls_opts) == int(out["sizeof"])
 
 
 def test_no_device_means_loud_failure_not_fallback():

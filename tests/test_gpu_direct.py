@@ -43,6 +43,32 @@ def test_direct_against_oracle_cfg2_offset_range_and_ragged_tail():
     assert np.max(np.abs(Pd[ks - k0] - oracle_power(w, ks=ks))) <= 1e-12
 
 
+def test_cfg3_nufft_power_against_direct_sums_through_the_oracles_assembly():
+    """ls_direct_power shares the K6 arithmetic (ls_power.cuh) with the NUFFT path, so an error there would cancel in
+    the comparison above.  Here the brute-force SUMS (ls_direct_sums: no assembly) go through the ORACLE's assembly, on
+    2^17 frequencies of config 3 across the mode-wrap seam: K6 of the NUFFT path is checked by independent code."""
+    import oracle
+    torch = require_cuda()
+    from paper_2409_08090_b200 import binding as B
+    w = make_workload(3)
+    Pg = gpu_power(w)[0]
+    dev = torch.device("cuda:0")
+    t = torch.from_numpy(w.t).to(dev); y = torch.from_numpy(np.ascontiguousarray(w.y[0])).to(dev)
+    dy = torch.from_numpy(w.dy).to(dev)
+    K = 1 << 17
+    k0 = w.Nf // 2 - K // 2
+    S = torch.empty((K, 6), dtype=torch.float64, device=dev)
+    B.ls_direct_sums(w.Nd, w.f0, w.df, k0, K, t, y, dy, S, torch.cuda.current_stream().cuda_stream)
+    sums = S.cpu().numpy()
+    ks = k0 + np.arange(0, K, 4096)
+    _, so, _ = oracle.direct(w.t, w.y[0], w.dy, w.f0, w.df, w.Nf, k=ks, return_sums=True)
+    assert np.max(np.abs(sums[ks - k0] - so)) <= 1e-13           # direct vs direct sums (|sums| <= 1)
+    _, _, YY = oracle.stats(w.y[0], w.dy)
+    Po = oracle.assemble(sums, YY)[0]
+    e = errors(Pg[k0:k0 + K], Po)
+    assert e["Einf"] <= GATE_F64 and e["median"] <= 1e-8 and e["p99"] <= 1e-6, e
+
+
 def test_direct_rejects_bad_arguments():
     require_cuda()
     from paper_2409_08090_b200 import binding as B

@@ -270,6 +270,49 @@ def test_plan_options(opts):
     _check64(e, pointwise=False)
 
 
+@pytest.mark.parametrize("tile", [256, 512, 1024])
+@pytest.mark.parametrize("p", [15, 20])
+def test_every_accepted_tile_length(tile, p):
+    """every tile_cells the plan accepts has an instantiated kernel, on the cuFFT path (forced), the small
+    own FFT (n = 2^15) and the pruned own FFT (n = 2^20: a pass-1 tile of 128 columns lies inside ONE spreading tile)."""
+    rng = np.random.default_rng(50 + p)
+    Nf = int(0.7 * (1 << p)); Nd = max(300, Nf // 10)
+    t = rng.uniform(0, 900.0, Nd); dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    y = np.sin(2 * np.pi * (df + (Nf // 3) * df) * t) + rng.normal(0, 1.0, Nd)
+    w = _custom(t, y, dy, df, df, Nf)
+    ks = compare_indices(w, 300)
+    Po = oracle_power(w, ks=ks)
+    for fft_impl in (0, 1):
+        Pg, ex = gpu_power(w, tile_cells=tile, no_autotune=1, fft_impl=fft_impl, return_plan_info=True)
+        assert ex["info"]["n"] == 1 << p
+        _check64(errors(Pg[0][ks], Po))
+    wb = Workload("tiles_batch", t, np.stack([y, 2 * y + 1]), dy, df, df, Nf, "f64", 1e-9)
+    if tile <= 512:
+        Pb = gpu_power(wb, tile_cells=tile, no_autotune=1)
+        assert np.max(np.abs(Pb[0][ks] - Po)) / Po.max() <= GATE_F64
+
+
+def test_rejected_tile_lengths_and_widths():
+    from gpu_util import require_cuda
+    require_cuda()
+    from paper_2409_08090_b200 import binding as B
+    for bad in (64, 128, 320, 768, 2048):
+        with pytest.raises(B.LsError) as ei:
+            B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 1, tile_cells=bad)
+        assert ei.value.code == 1, bad
+    with pytest.raises(B.LsError) as ei:
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-9, B.LS_F64, 2, tile_cells=1024)      # a batch has two cells per thread
+    assert ei.value.code == 1
+    # eps = 1e-13 at sigma = 1.25 needs more than the 20 cells the kernels hold: refused, not silently clamped ...
+    with pytest.raises(B.LsError) as ei:
+        B.Plan(1000, 12500, 0.1, 0.1, 1e-13, B.LS_F64, 1, upsampfac=1.25)
+    assert ei.value.code == 5
+    # ... and in automatic mode the grid doubles instead (Nf = 12 500: 2^14 has sigma 1.31, needs 25 cells)
+    with B.Plan(1000, 12500, 0.1, 0.1, 1e-13, B.LS_F64, 1) as plan:
+        assert plan.info["n"] == 1 << 15 and plan.info["w"] <= 20
+
+
 def test_batch_chunking_matches_single_pass():
     w = scaled_workload(4, 1500, batch=11)
     P_one = gpu_power(w, batch_chunk=11)
