@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--cpu-freqs", type=int, default=0, help="oracle sample size (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (tuning runs)")
+    ap.add_argument("--parity-k", type=int, default=64, help="frequencies of the timed plan's output checked against "
+                    "the oracle after the timed loop (0 = skip)")
     # plan tuning knobs (ls_opts); 0 = the library's automatic choice
     ap.add_argument("--tile-cells", type=int, default=0)
     ap.add_argument("--upsampfac", type=float, default=0.0)
@@ -440,6 +442,27 @@ def run_ours(args):
         "gpu_launches": own * args.steps, "own_kernels_per_step": own, "cufft_execs_per_step": ffts,
         "clocks": clocks,
     }
+    if args.parity_k > 0:
+        # The output of the plan that was TIMED (same launch configuration: side stream, graph replay), checked after the
+        # timed loop against the oracle's direct sums on sampled frequencies (peak and seam included): the paper's error
+        # metric (pointwise relative error, median / 99th percentile) next to the gate's E_inf (A8).
+        import oracle
+        from paper_2409_08090_b200.workloads import compare_indices
+        P.fill_(float("nan"))
+        with torch.cuda.stream(side):
+            plan.execute(t, y, dy, P, stream)
+        side.synchronize()
+        ks = compare_indices(w, args.parity_k)
+        nser = min(w.batch, 2)
+        Pg = P[:nser].cpu().numpy().astype(np.float64)[:, ks]
+        Po = np.stack([oracle.direct(w.t, w.y[b], w.dy, w.f0, w.df, w.Nf, k=ks) for b in range(nser)])
+        d = np.abs(Pg - Po)
+        rel = d / np.maximum(Po, 1e-300)
+        gate = 1e-8 if w.dtype == "f64" else 1e-4
+        line["parity"] = {"against": "oracle.direct (strict)", "K": int(ks.size), "series": nser,
+                          "Einf": float((d.max(axis=1) / Po.max(axis=1)).max()), "median": float(np.median(rel)),
+                          "p99": float(np.percentile(rel, 99)), "max": float(rel.max()), "gate_Einf": gate,
+                          "ok": bool((d.max(axis=1) / Po.max(axis=1)).max() <= gate and np.all(np.isfinite(Pg)))}
     if not args.no_cpu_baseline and world == 1:
         import oracle
         cores = oracle.num_threads()
