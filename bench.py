@@ -59,6 +59,10 @@ def parse_args():
     ap.add_argument("--batch-chunk", type=int, default=0)
     ap.add_argument("--fft-impl", type=int, default=0, help="0 auto, 1 cuFFT, 2 own FFT with the last pass fused into the assembly, 3 own FFT unfused")
     ap.add_argument("--graph", type=int, default=0, help="0 auto, 1 never, 2 always (user-facing plan)")
+    ap.add_argument("--traffic-from", default="", help="CPU-side helper: turn `ncu -i REP --page raw --csv` output into "
+                    "profiles/r2_traffic.csv (needs --traffic-meta workload,n,w and --traffic-command)")
+    ap.add_argument("--traffic-meta", default="cfg3_single_Nd1e6_f64,16777216,17")
+    ap.add_argument("--traffic-command", default="")
     ap.add_argument("--variant", type=int, default=0, help="ls_opts.reserved[0]: kernel variant kept for comparison")
     ap.add_argument("--lag", type=int, default=0, help="ls_opts.reserved[1]: queue lag of the fused FFT kernels (0 = default)")
     return ap.parse_args()
@@ -255,22 +259,77 @@ def stage_model_bytes(w, info, own_fft, L):
     return d
 
 
+TRAFFIC_FILE = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+KERNEL_STAGE = {"ls_stats_count_kernel": "stats", "ls_premultiply_kernel": "premul", "ls_spread_tile_kernel": "spread",
+                "ls_fft_pass1_kernel": "fft_pass1", "ls_fft_pass23_tma_kernel": "fft_pass23", "ls_fft_pass23_kernel": "fft_pass23",
+                "ls_assemble_kernel": "assemble", "ls_assemble_shared_kernel": "assemble", "ls_fft_cols_kernel": "fft_pass2",
+                "ls_fft_rows_kernel": "fft_pass3", "ls_bin_scan_totals_kernel": "sort", "ls_bin_scan_apply_kernel": "sort",
+                "ls_tile_list_kernel": "sort", "ls_rows_kernel": "premul"}
+
+
+def source_hash():
+    """sha256 prefix over the library's CUDA sources: ties a committed ncu capture to the kernels it measured."""
+    import glob, hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_2409_08090_b200", "csrc")
+    for f in sorted(glob.glob(os.path.join(csrc, "*.cu")) + glob.glob(os.path.join(csrc, "*.cuh")) + glob.glob(os.path.join(csrc, "*.h"))):
+        with open(f, "rb") as fh:
+            h.update(os.path.basename(f).encode() + b"\0" + fh.read())
+    return h.hexdigest()[:16]
+
+
+def write_traffic(raw_csv, meta, command):
+    """`ncu -i X.ncu-rep --page raw --csv` output -> profiles/r2_traffic.csv (per-launch means of every own kernel),
+    stamped with the hash of the sources it was captured from.  Runs on the CPU box; no GPU needed."""
+    import csv
+    workload, n, wd = meta.split(",")
+    with open(raw_csv) as f:
+        rows = list(csv.reader(f))
+    hdr = rows[0]
+    ik, it = hdr.index("Kernel Name"), hdr.index("gpu__time_duration.sum")
+    ir, iw = hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    units = rows[1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "ns": 1e-3, "us": 1.0, "ms": 1e3, "usecond": 1.0, "nsecond": 1e-3, "msecond": 1e3}
+    acc = {}
+    for r in rows[2:]:
+        name = next((k for k in KERNEL_STAGE if k in r[ik]), None)
+        if name is None:
+            continue
+        a = acc.setdefault(name, [0, 0.0, 0.0, 0.0])
+        a[0] += 1
+        a[1] += float(r[it].replace(",", "")) * scale[units[it]]
+        a[2] += float(r[ir].replace(",", "")) * scale[units[ir]]
+        a[3] += float(r[iw].replace(",", "")) * scale[units[iw]]
+    with open(TRAFFIC_FILE, "w") as f:
+        f.write("# dram__bytes_read.sum / dram__bytes_write.sum per launch (mean over the captured launches) of every own kernel\n")
+        f.write(f"# command: {command}\n")
+        f.write(f"# source_hash: {source_hash()}\n")
+        f.write("stage,kernel,workload,n,w,launches,time_us,dram_read_bytes,dram_write_bytes\n")
+        for name, a in acc.items():
+            f.write(f"{KERNEL_STAGE[name]},{name},{workload},{n},{wd},{a[0]},{a[1] / a[0]:.1f},{a[2] / a[0]:.0f},{a[3] / a[0]:.0f}\n")
+    print(f"wrote {TRAFFIC_FILE} ({len(acc)} kernels, source_hash {source_hash()})")
+
+
 def measured_traffic(kernel_stage, w, info):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernel, from the committed
-    ncu --set full capture (profiles/r1j_traffic.csv; same command line, config 3 defaults).  None when
-    the capture does not cover this workload / plan."""
-    path = os.path.join(ROOT, "profiles", "r1j_traffic.csv")
+    """(dram__bytes_read.sum + dram__bytes_write.sum per launch of the stage's kernels, capture record) from the
+    committed ncu --set full capture profiles/r2_traffic.csv; the record says which sources the capture saw and whether
+    they are the sources of this run (`stale`).  (None, None) when the capture does not cover this workload / plan."""
     try:
-        with open(path) as f:
-            rows = [l.strip().split(",") for l in f if l.strip() and not l.startswith("#")]
+        with open(TRAFFIC_FILE) as f:
+            lines = [l.strip() for l in f if l.strip()]
+        cap_hash = next((l.split(":", 1)[1].strip() for l in lines if l.startswith("# source_hash:")), None)
+        rows = [l.split(",") for l in lines if not l.startswith("#")]
         hdr, rows = rows[0], rows[1:]
+        tot = None
         for r in rows:
             d = dict(zip(hdr, r))
             if d["stage"] == kernel_stage and d["workload"] == w.name and int(d["n"]) == info["n"] and int(d["w"]) == info["w"]:
-                return float(d["dram_read_bytes"]) + float(d["dram_write_bytes"])
+                tot = (tot or 0.0) + float(d["dram_read_bytes"]) + float(d["dram_write_bytes"])
+        if tot is None:
+            return None, None
+        return tot, {"file": "profiles/r2_traffic.csv", "source_hash": cap_hash, "stale": cap_hash != source_hash()}
     except Exception:
-        pass
-    return None
+        return None, None
 
 
 def run_ours(args):
@@ -401,6 +460,7 @@ def run_ours(args):
     path_ms = stage["total"] - stage["fft"]
     path_ach = info["model_bytes"] / (path_ms * 1e-3) / 1e9
     path_sparse = info["model_bytes"] - (info["M"] * info["n"] * 2 * (8 if w.dtype == "f64" else 4) - (sbytes["spread"] - 2 * w.Nd * 4 * (8 if w.dtype == "f64" else 4) - info["M"] * w.Nd * (8 if w.dtype == "f64" else 4)))
+    traffic, traffic_cap = measured_traffic(dom, w, info)
     Bi = ht.numel() * ht.element_size() + hy.numel() * hy.element_size() + hdy.numel() * hdy.element_size()
     Bo = hP.numel() * hP.element_size()
     line = {
@@ -414,7 +474,7 @@ def run_ours(args):
         "stage_ms": stage, "wall_ms_per_step_incl_flush": wall / args.steps * 1e3,
         "step_ms_min": float(np.min(step_ms)), "step_ms_median": float(np.median(step_ms)),
         "roofline": {"bound": "hbm", "kernel": dom, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                     "traffic": measured_traffic(dom, w, info), "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
+                     "traffic": traffic, "traffic_capture": traffic_cap, "peak_source": peak_src, "algorithmic_bytes": sbytes[dom],
                      "kernel_ms": stage[dom],
                      "per_kernel": {k: {"ms": stage[k], "algorithmic_bytes": sbytes[k],
                                         "frac": sbytes[k] / (stage[k] * 1e-3) / 1e9 / peak if stage[k] > 0 else None}
@@ -480,7 +540,9 @@ def run_ours(args):
 
 if __name__ == "__main__":
     a = parse_args()
-    if a.impl == "reference":
+    if a.traffic_from:
+        write_traffic(a.traffic_from, a.traffic_meta, a.traffic_command)
+    elif a.impl == "reference":
         run_reference(a)
     else:
         run_ours(a)
