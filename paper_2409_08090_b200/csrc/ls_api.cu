@@ -224,9 +224,12 @@ void build_passes(const ls_plan_s* p, std::vector<Pass>& out) {
         Pass ps;
         ps.s0 = s0;
         ps.C = std::min(p->chunk, p->batch - s0);
-        if (per) { ps.fft_slot0 = 0; ps.fft_batch = 3 * ps.C; }
-        else if (s0 == 0) { ps.fft_slot0 = 0; ps.fft_batch = 2 + ps.C; }
-        else { ps.fft_slot0 = 2; ps.fft_batch = ps.C; }
+        // fixed mean (opts.no_floating_mean): the w transform at x1 is not needed — the paper's "pair of NUFFTs"
+        // (PAPER.md:17): w at x2 and h at x1 only
+        const int nw = p->opts.no_floating_mean ? 0 : 1;
+        if (per) { ps.fft_slot0 = 0; ps.fft_batch = (2 + nw) * ps.C; }
+        else if (s0 == 0) { ps.fft_slot0 = 0; ps.fft_batch = 1 + nw + ps.C; }
+        else { ps.fft_slot0 = 1 + nw; ps.fft_batch = ps.C; }
         out.push_back(ps);
     }
 }
@@ -378,7 +381,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         int64_t m = 64;                                 // >= 2 kMaxWidth
         while ((double)m < want) m *= 2;
         p->n = m;
-        const int ntrans = o.dy_per_series ? 3 * batch : batch + 2;
+        const int ntrans = (o.dy_per_series ? 3 * batch : batch + 2) - (o.no_floating_mean ? (o.dy_per_series ? batch : 1) : 0);
         if ((double)m > 1.6 * (double)Nf && (double)m * ntrans >= (double)((int64_t)1 << 20) && !o.no_autotune) {
             // the timed choice is cached per (Nf, dtype, transforms, device): the same arguments give the same grid — and
             // therefore the same results — for the life of the process (between processes it may differ: ls.h)
@@ -430,7 +433,8 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         p->tile_stride = (int)(st % p->ntiles == 0 ? 1 : st % p->ntiles);
     }
     const bool per = o.dy_per_series != 0;
-    p->M = per ? 3 * batch : batch + 2;
+    const int nw = o.no_floating_mean ? 0 : 1;     // the w transform at x1 exists only with the floating mean
+    p->M = per ? (2 + nw) * batch : batch + 1 + nw;
     const size_t B = real_bytes(dtype);
     const size_t grid_bytes = (size_t)p->n * 2 * B;
     if (o.batch_chunk > 0) p->chunk = std::min(o.batch_chunk, batch);
@@ -440,7 +444,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         // series with 64 MB chunks, 5.3 ms in one pass).  So: as many series per pass as 8 GB of grids hold.
         p->chunk = (int)std::max<size_t>(1, std::min<size_t>((size_t)batch, ((size_t)8 << 30) / grid_bytes));
     }
-    p->slots = per ? 3 * p->chunk : 2 + p->chunk;
+    p->slots = per ? (2 + nw) * p->chunk : 1 + nw + p->chunk;
 
     // own FFT: wherever it exists when asked for (fft_impl 2, 3); in auto mode for the pruned sizes (n >= 2^20) and, below
     // them, for problems small enough to be latency-bound (cuFFT runs a 2^14-point fp64 transform in ONE CTA: 29 us of
@@ -502,7 +506,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         for (int i = 0; i < 2 && ce == cudaSuccess; ++i) {
             lsb::PointSet& ps = p->ps[i];
             // stored strength rows (shared dy: the weights live in the records, only y - ybar is stored)
-            ps.nrows = i == 0 ? (per ? 2 * batch : batch) : (per ? batch : 0);
+            ps.nrows = i == 0 ? (per ? (1 + nw) * batch : batch) : (per ? batch : 0);
             if ((ce = dmalloc(p, &ps.bin_start, (size_t)(p->nbins + 1) * 4)) != cudaSuccess) break;
             if ((batch > 1 || per) && (ce = dmalloc(p, &ps.perm, (size_t)Nd * 4)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&ps.rec, (size_t)Nd * 4 * B)) != cudaSuccess) break;
@@ -604,16 +608,20 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
         for (const Pass& ps : passes) {
             int h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride;
             stage_begin(p, LS_STAGE_SPREAD, s);
+            const int nw = p->opts.no_floating_mean ? 0 : 1;
             if (per) {
-                // slots [0, C): w2_s ; slots [C, 3C): (w_s, h_s) pairs
-                LS_TRY(lsb::launch_spread(p, ps.s0, ps.C, 0, 2 * ps.s0, 2 * ps.C, ps.C, s)); ++own;
-                w2_slot = 0; w2_stride = 1; w_slot = ps.C; w_stride = 2; h_slot = ps.C + 1; h_stride = 2;
+                // slots [0, C): w2_s ; slots [C, 3C): (w_s, h_s) pairs — fixed mean: [C, 2C): h_s (the rows kernel then
+                // stores the h rows only)
+                LS_TRY(lsb::launch_spread(p, ps.s0, ps.C, 0, (1 + nw) * ps.s0, (1 + nw) * ps.C, ps.C, s)); ++own;
+                w2_slot = 0; w2_stride = 1; h_slot = ps.C + nw; h_stride = 1 + nw;
+                w_slot = nw ? ps.C : 0; w_stride = nw ? 2 : 1;                 // fixed mean: unused (x 0): any finite modes
             } else {
-                // slot 0: w2, slot 1: w, slots 2..: h_s of this pass
-                if (ps.s0 == 0) LS_TRY(lsb::launch_spread(p, 0, 1, 0, 0, 1 + ps.C, 1, s));
-                else LS_TRY(lsb::launch_spread(p, 0, 0, 0, 1 + ps.s0, ps.C, 2, s));
+                // slot 0: w2, slot 1: w, slots 2..: h_s of this pass — fixed mean: slot 0: w2, slots 1..: h_s (logical row 0
+                // of the x1 point set, the w transform, is skipped)
+                if (ps.s0 == 0) LS_TRY(lsb::launch_spread(p, 0, 1, 0, 1 - nw, nw + ps.C, 1, s));
+                else LS_TRY(lsb::launch_spread(p, 0, 0, 0, 1 + ps.s0, ps.C, 1 + nw, s));
                 ++own;
-                w2_slot = 0; w2_stride = 0; w_slot = 1; w_stride = 0; h_slot = 2; h_stride = 1;
+                w2_slot = 0; w2_stride = 0; w_slot = nw; w_stride = 0; h_slot = 1 + nw; h_stride = 1;
             }
             stage_end(p, s);
             if (p->debug_stop_after_spread) break;      // ls_debug_grid: the fine grids as the spreading kernel left them
@@ -622,7 +630,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 // own three-pass FFT: pass 1 skips the tiles spreading left unwritten; pass 3 emits compact modes
                 // (fused mode: only of w2, w — the h transforms' pass 3 is part of the assembly kernel below)
                 const int n_x2 = per ? ps.C : (ps.s0 == 0 ? 1 : 0);
-                const int n_modes = !p->fuse_assemble ? ps.fft_batch : (ps.s0 == 0 ? 2 : 0);
+                const int n_modes = !p->fuse_assemble ? ps.fft_batch : (ps.s0 == 0 ? 1 + nw : 0);
                 stage_begin(p, LS_STAGE_FFT_PASS1, s);
                 LS_TRY(lsb::launch_own_fft_pass1(p, ps.fft_slot0, ps.fft_batch, n_x2, s));
                 stage_end(p, s);
@@ -833,9 +841,10 @@ int ls_debug_modes(ls_plan_t p, int series, int64_t K, const int64_t* kidx, doub
         if (kidx[i] < 0 || kidx[i] >= p->Nf) return LS_ERR_INVALID_VALUE;
     const bool per = p->opts.dy_per_series != 0;
     const int C = p->batch;
-    const int h_slot = per ? C + 2 * series + 1 : 2 + series;
-    const int w_slot = per ? C + 2 * series : 1;
+    const int nw = p->opts.no_floating_mean ? 0 : 1;
     const int w2_slot = per ? series : 0;
+    const int h_slot = per ? C + (1 + nw) * series + nw : 1 + nw + series;
+    const int w_slot = !nw ? w2_slot : (per ? C + 2 * series : 1);     // fixed mean: no w transform (reported as w2's)
     int64_t* dk = nullptr;
     double* dout = nullptr;
     int rc = LS_OK;

@@ -343,7 +343,7 @@ ls_premultiply_kernel(const double* __restrict__ t, const T* __restrict__ y, con
 template <typename T>
 __global__ void __launch_bounds__(kPreThreads)
 ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __restrict__ sums,
-               long long Nd, int dy_per_series, const int* __restrict__ perm1,
+               long long Nd, int dy_per_series, int no_w_row, const int* __restrict__ perm1,
                const int* __restrict__ perm2, T* __restrict__ R1, T* __restrict__ R2) {
     __shared__ double red[kPreThreads / 32];
     const int s = blockIdx.y;
@@ -354,7 +354,8 @@ ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __rest
     const double invW = 1.0 / W;
     // per-series dy: R1 = [w_0, h_0, w_1, h_1, ...], R2 = [w_0, w_1, ...], h_s = w_s (y_s - ybar_s);
     // shared dy (weights folded into the records' phasors): R1 = [y_0 - ybar_0, y_1 - ybar_1, ...], no R2
-    T* rowh = R1 + (long long)(dy_per_series ? 2 * s + 1 : s) * Nd;
+    // (fixed mean, no_w_row: the w transform at x1 does not exist and its row is not stored: R1 = [h_0, h_1, ...])
+    T* rowh = R1 + (long long)((dy_per_series && !no_w_row) ? 2 * s + 1 : s) * Nd;
     T* roww1 = R1 + (long long)(2 * s) * Nd;
     T* roww2 = R2 + (long long)s * Nd;
     double yy = 0.0;
@@ -367,7 +368,7 @@ ls_rows_kernel(const T* __restrict__ y, const T* __restrict__ dy, double* __rest
         yy += wj * yc * yc;
         if (dy_per_series) {
             rowh[q] = (T)(wj * yc);
-            roww1[q] = (T)wj;
+            if (!no_w_row) roww1[q] = (T)wj;
             const double d2 = (double)ds[perm2[q]];
             roww2[q] = (T)(invW / (d2 * d2));
         } else {
@@ -448,12 +449,12 @@ cudaError_t launch_rows(ls_plan_s* p, const void* y, const void* dy, cudaStream_
     dim3 grid(point_blocks(p->Nd, p->batch), p->batch);
     if (p->dtype == LS_F64)
         ls_rows_kernel<double><<<grid, kPreThreads, 0, s>>>((const double*)y, (const double*)dy, p->sums, p->Nd,
-                                                            p->opts.dy_per_series, p->ps[0].perm, p->ps[1].perm,
-                                                            (double*)p->ps[0].rows, (double*)p->ps[1].rows);
+                                                            p->opts.dy_per_series, p->opts.no_floating_mean, p->ps[0].perm,
+                                                            p->ps[1].perm, (double*)p->ps[0].rows, (double*)p->ps[1].rows);
     else
         ls_rows_kernel<float><<<grid, kPreThreads, 0, s>>>((const float*)y, (const float*)dy, p->sums, p->Nd,
-                                                           p->opts.dy_per_series, p->ps[0].perm, p->ps[1].perm,
-                                                           (float*)p->ps[0].rows, (float*)p->ps[1].rows);
+                                                           p->opts.dy_per_series, p->opts.no_floating_mean, p->ps[0].perm,
+                                                           p->ps[1].perm, (float*)p->ps[0].rows, (float*)p->ps[1].rows);
     return cudaGetLastError();
 }
 

@@ -53,6 +53,32 @@ def test_variants_batch_shared_and_per_series_dy():
             assert _rel(Pg[b], Po) <= 1e-8, (per, b)
 
 
+def test_fixed_mean_is_a_pair_of_transforms():
+    """opts.no_floating_mean runs the paper's "pair of NUFFTs": w at x2 and h at x1 — the w transform at
+    x1 is neither spread nor transformed (M = batch + 1 with shared dy, 2 batch with per-series dy); batch passes,
+    the fused last pass and the mode debug hook keep working on the shorter slot layout."""
+    import oracle
+    w = scaled_workload(4, 1500, batch=5)
+    for chunk in (0, 2):
+        Pg, ex = gpu_power(w, no_floating_mean=1, batch_chunk=chunk, return_plan_info=True,
+                           debug_modes=(3, np.arange(0, w.Nf, 7)) if chunk == 0 else None)
+        assert ex["info"]["M"] == 6
+        for b in (0, 3, 4):
+            Po = variants.power(w.t, w.y[b], w.dy, w.f0, w.df, w.Nf, fit_mean=False)
+            assert _rel(Pg[b], Po) <= 1e-8, (chunk, b)
+        if chunk == 0:
+            _, sums, _ = oracle.direct(w.t, w.y[3], w.dy, w.f0, w.df, w.Nf, k=np.arange(0, w.Nf, 7), return_sums=True)
+            g = ex["modes"]
+            assert np.max(np.abs(g[:, [0, 1, 4, 5]] - sums[:, [0, 1, 4, 5]])) <= 1e-9       # (Sh, Ch) and (S2, C2)
+    wp = scaled_workload(4, 1500, batch=3)
+    wp.dy = np.ascontiguousarray(np.random.default_rng(6).uniform(0.5, 1.5, (3, wp.Nd)))
+    Pg, ex = gpu_power(wp, no_floating_mean=1, return_plan_info=True)
+    assert ex["info"]["M"] == 6
+    for b in range(3):
+        assert _rel(Pg[b], variants.power(wp.t, wp.y[b], wp.dy[b], wp.f0, wp.df, wp.Nf, fit_mean=False)) <= 1e-8
+    assert gpu_power(scaled_workload(2, 2000), no_floating_mean=1, return_plan_info=True)[1]["info"]["M"] == 2
+
+
 def test_astropy_style_front_end():
     import torch
     from paper_2409_08090_b200.lombscargle import LombScargle
