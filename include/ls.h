@@ -193,13 +193,17 @@ int ls_debug_stats(ls_plan_t plan, double* out);
  *   ls_debug_grid: runs K1..K4 on (t, y, dy) (device pointers, legacy stream) and returns fine grid `slot` as the
  *     spreading kernel left it: out[n][2].  LS_ERR_UNSUPPORTED where empty tiles are not written (own FFT, n >= 2^20).
  *   ls_debug_dinv: out[i] = 1 / psihat(k') at |k'| = kabs[i] <= Nf / 2 (the P0 table).
- *   ls_debug_assemble: K6 alone (no plan): power of K frequencies from sums[K][6] = (Sh, Ch, S, C, S2, C2). */
+ *   ls_debug_assemble: K6 alone (no plan): power of K frequencies from sums[K][6] = (Sh, Ch, S, C, S2, C2).
+ *   ls_debug_guards: with the environment variable LS_B200_GUARD set when the plan was made, every plan-owned device
+ *     allocation sits between two 256-byte guard zones; returns how many guard bytes any kernel has overwritten since
+ *     (0 = no out-of-bounds write).  LS_ERR_NOT_READY for a plan made without the variable. */
 int ls_debug_points(ls_plan_t plan, int set, double* out);
 int ls_debug_bins(ls_plan_t plan, int set, int* out);
 int ls_debug_grid(ls_plan_t plan, const void* t, const void* y, const void* dy, int slot, double* out);
 int ls_debug_dinv(ls_plan_t plan, int64_t K, const int64_t* kabs, double* out);
 int ls_debug_assemble(int64_t K, const double* sums, double YY, double W, int no_floating_mean, int normalization,
                       double* out);
+int ls_debug_guards(ls_plan_t plan, int64_t* damaged_bytes);
 
 /* ls_direct_power — verification path, NOT part of ls_execute: the six sums of
  * Eq. 1 evaluated by brute force, O(Nd K), for the K consecutive frequencies

@@ -15,7 +15,7 @@ __all__ = [
     "LS_F32", "LS_F64", "LS_OK", "STAGES", "LsError", "ls_opts", "lib_path", "load",
     "ls_plan", "ls_execute", "ls_execute_host", "ls_destroy", "ls_get_info", "ls_workspace_bytes", "ls_set_workspace",
     "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_debug_points", "ls_debug_bins", "ls_debug_grid", "ls_debug_dinv",
-    "ls_debug_assemble", "ls_strerror", "ls_direct_power", "ls_direct_sums",
+    "ls_debug_assemble", "ls_debug_guards", "ls_strerror", "ls_direct_power", "ls_direct_sums",
     "exported_symbols", "Plan",
 ]
 
@@ -73,6 +73,7 @@ _SIGNATURES = {
     "ls_debug_bins": (C.c_int, [C.c_void_p, C.c_int, C.POINTER(C.c_int)]),
     "ls_debug_grid": (C.c_int, [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int, C.POINTER(C.c_double)]),
     "ls_debug_dinv": (C.c_int, [C.c_void_p, C.c_int64, C.POINTER(C.c_int64), C.POINTER(C.c_double)]),
+    "ls_debug_guards": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
     "ls_debug_assemble": (C.c_int, [C.c_int64, C.POINTER(C.c_double), C.c_double, C.c_double, C.c_int, C.c_int,
                                     C.POINTER(C.c_double)]),
     "ls_direct_power": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
@@ -264,6 +265,15 @@ def ls_debug_dinv(plan, kabs):
     if rc != LS_OK:
         raise LsError(rc, "ls_debug_dinv")
     return out
+
+
+def ls_debug_guards(plan) -> int:
+    """Guard-zone bytes overwritten by any kernel since the plan was made (needs LS_B200_GUARD in the environment)."""
+    n = C.c_int64()
+    rc = load().ls_debug_guards(plan, C.byref(n))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_debug_guards")
+    return int(n.value)
 
 
 def ls_debug_assemble(sums, YY, W=1.0, no_floating_mean=0, normalization=0):

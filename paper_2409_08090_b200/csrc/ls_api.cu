@@ -209,12 +209,36 @@ int64_t autotune_grid_size(int64_t Nf, int dtype, int64_t n_pow2, int ntrans) {
     return best;
 }
 
+// Plan-owned device memory.  With the environment variable LS_B200_GUARD set when the plan is made, every allocation
+// is wrapped in two 256-byte guard zones filled with 0xA5 that ls_debug_guards checks: an out-of-bounds WRITE of any
+// kernel shows up as a damaged guard (compute-sanitizer is closed on this GPU pool, profiles/r2_checks.md).
+constexpr size_t kGuardBytes = 256;
 template <typename T>
 cudaError_t dmalloc(ls_plan_s* p, T** ptr, size_t bytes) {
     if (bytes == 0) bytes = 16;
-    cudaError_t e = cudaMalloc((void**)ptr, bytes);
-    if (e == cudaSuccess) p->total_bytes += bytes;
-    return e;
+    const size_t g = p->guard ? kGuardBytes : 0;
+    char* base = nullptr;
+    cudaError_t e = cudaMalloc((void**)&base, bytes + 2 * g);
+    if (e != cudaSuccess) return e;
+    if (g) {
+        if ((e = cudaMemset(base, 0xA5, g)) != cudaSuccess || (e = cudaMemset(base + g + bytes, 0xA5, g)) != cudaSuccess) return e;
+        p->guards.push_back({base, bytes});
+    }
+    p->total_bytes += bytes;
+    *ptr = (T*)(base + g);
+    return cudaSuccess;
+}
+void dfree(ls_plan_s* p, void* ptr) {
+    if (!ptr) return;
+    if (p->guard) {
+        for (auto& gz : p->guards)
+            if (gz.first && gz.first + kGuardBytes == (char*)ptr) {
+                cudaFree(gz.first);
+                gz.first = nullptr;
+                return;
+            }
+    }
+    cudaFree(ptr);
 }
 
 void build_passes(const ls_plan_s* p, std::vector<Pass>& out) {
@@ -300,27 +324,27 @@ int ls_destroy(ls_plan_t p) {
     if (p->has_chunk) cufftDestroy(p->fft_chunk);
     if (p->has_rem) cufftDestroy(p->fft_rem);
     if (!p->external_ws) {
-        cudaFree(p->fft_work);
-        cudaFree(p->grids);
-        cudaFree(p->modes);
+        dfree(p, p->fft_work);
+        dfree(p, p->grids);
+        dfree(p, p->modes);
     }
-    cudaFree(p->dinv);
-    cudaFree(p->t64);
-    cudaFree(p->fft_wlo);
-    cudaFree(p->fft_whi);
-    cudaFree(p->tile_list);
-    cudaFree(p->zeroed);                     // sums and both histograms live in this allocation
-    cudaFree(p->scan_tmp);
+    dfree(p, p->dinv);
+    dfree(p, p->t64);
+    dfree(p, p->fft_wlo);
+    dfree(p, p->fft_whi);
+    dfree(p, p->tile_list);
+    dfree(p, p->zeroed);                     // sums and both histograms live in this allocation
+    dfree(p, p->scan_tmp);
     for (int i = 0; i < 2; ++i) {
-        cudaFree(p->ps[i].bin_start);
-        cudaFree(p->ps[i].perm);
-        cudaFree(p->ps[i].rec);
-        cudaFree(p->ps[i].rows);
+        dfree(p, p->ps[i].bin_start);
+        dfree(p, p->ps[i].perm);
+        dfree(p, p->ps[i].rec);
+        dfree(p, p->ps[i].rows);
     }
-    cudaFree(p->st_t);
-    cudaFree(p->st_y);
-    cudaFree(p->st_dy);
-    cudaFree(p->st_p);
+    dfree(p, p->st_t);
+    dfree(p, p->st_y);
+    dfree(p, p->st_dy);
+    dfree(p, p->st_p);
     for (auto& ev : p->events) {
         cudaEventDestroy(ev.beg);
         cudaEventDestroy(ev.end);
@@ -361,6 +385,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     ls_plan_s* p = new (std::nothrow) ls_plan_s;
     if (!p) return LS_ERR_ALLOC;
     p->Nd = Nd; p->Nf = Nf; p->f0 = f0; p->df = df; p->eps = eps; p->dtype = dtype; p->batch = batch;
+    p->guard = getenv("LS_B200_GUARD") != nullptr;
     p->opts = o;
     if (cudaDeviceGetAttribute(&p->num_sms, cudaDevAttrMultiProcessorCount, o.device) != cudaSuccess || p->num_sms < 1) {
         cudaGetLastError();
@@ -773,9 +798,9 @@ int ls_set_workspace(ls_plan_t p, void* dptr, size_t bytes) {
         return LS_ERR_CUDA;
     }
     if (!p->external_ws) {
-        cudaFree(p->grids);
-        cudaFree(p->modes);
-        cudaFree(p->fft_work);
+        dfree(p, p->grids);
+        dfree(p, p->modes);
+        dfree(p, p->fft_work);
     }
     char* base = (char*)dptr;
     p->grids = base;
@@ -930,6 +955,24 @@ int ls_debug_assemble(int64_t K, const double* sums, double YY, double W, int no
     cudaFree(dout);
     if (rc != LS_OK) cudaGetLastError();
     return rc;
+}
+
+int ls_debug_guards(ls_plan_t p, int64_t* damaged_bytes) {
+    if (!p || !damaged_bytes) return LS_ERR_INVALID_VALUE;
+    if (!p->guard) return LS_ERR_NOT_READY;
+    if (cudaDeviceSynchronize() != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+    int64_t bad = 0;
+    unsigned char h[kGuardBytes];
+    for (const auto& gz : p->guards) {
+        if (!gz.first) continue;
+        for (int side = 0; side < 2; ++side) {
+            const char* src = gz.first + (side ? kGuardBytes + gz.second : 0);
+            if (cudaMemcpy(h, src, kGuardBytes, cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return LS_ERR_CUDA; }
+            for (size_t i = 0; i < kGuardBytes; ++i) bad += h[i] != 0xA5;
+        }
+    }
+    *damaged_bytes = bad;
+    return LS_OK;
 }
 
 }  // extern "C"

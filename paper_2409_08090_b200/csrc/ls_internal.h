@@ -8,6 +8,7 @@
 #include <stdint.h>
 
 #include <algorithm>
+#include <utility>
 #include <vector>
 
 #include "../../include/ls.h"
@@ -133,6 +134,8 @@ struct ls_plan_s {
     bool timed_once = false;
     int own_kernels = 0, fft_execs = 0;
     bool debug_stop_after_spread = false;   // ls_debug_grid
+    bool guard = false;                     // LS_B200_GUARD: allocations carry guard zones (ls_debug_guards)
+    std::vector<std::pair<char*, size_t>> guards;   // (base of the guarded allocation, payload bytes)
     double model_bytes = 0;
 };
 
