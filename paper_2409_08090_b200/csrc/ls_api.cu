@@ -477,6 +477,11 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     p->own_fft = o.fft_impl != 1 && lsb::own_fft_supported(p);
     if (p->own_fft && o.fft_impl == 0 && !lsb::own_fft_prunes(p) && (double)p->M * (double)p->n * 16.0 > 64e6) p->own_fft = false;
     p->fft_prune = p->own_fft && lsb::own_fft_prunes(p);
+    // cuFFT path, few transforms over very many tiles (config 5: 3 x 154 000): one sweep kernel zero-fills the empty tiles
+    // and lists the occupied ones for a persistent spreading launch.  Measured: config 5 spread 1.51 -> 1.34 ms; config 4
+    // (1002 transforms over 313 tiles) 0.54 -> 0.78 ms, so batches keep one CTA per (tile, row group).
+    // (reserved[0] = 1: never)
+    p->list_tiles = !p->own_fft && o.reserved[0] != 1 && ((p->M <= 8 && p->ntiles >= 32 * p->num_sms) || o.reserved[0] == 2);   // 2: always (tests)
     if (o.fft_impl >= 2 && !p->own_fft) { delete p; return LS_ERR_UNSUPPORTED; }
     // Measured at config 3 (profiles/r1e_cfg3.md): with the cheaper assembly arithmetic the separate
     // assembly kernel (0.118 ms at 81 % of DRAM peak) plus an unfused third pass beats the fused kernel, which is
@@ -512,14 +517,14 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
-        const size_t mask_bytes = p->fft_prune ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : 0;   // masks + 2 list counters
+        const size_t mask_bytes = p->fft_prune ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : (p->list_tiles ? 256 : 0);   // masks + 2 list counters
         const size_t queue_bytes = p->fft_prune ? (((size_t)(2 + 32 * p->slots) * 4 + 255) & ~(size_t)255) : 0;
         p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes + queue_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
         if (queue_bytes) p->fft_queue = (int*)((char*)p->zeroed + sums_bytes + hist_bytes + mask_bytes);
-        if (p->fft_prune) {
+        if (p->fft_prune || p->list_tiles) {
             p->tile_counts = (int*)((char*)p->zeroed + sums_bytes + hist_bytes);
-            p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes + 256);
+            if (p->fft_prune) p->row_masks = (unsigned*)((char*)p->zeroed + sums_bytes + hist_bytes + 256);
             if ((ce = dmalloc(p, &p->tile_list, (size_t)2 * p->ntiles * 4)) != cudaSuccess) break;
         }
         p->sums = (double*)p->zeroed;
@@ -634,6 +639,12 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
             int h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride;
             stage_begin(p, LS_STAGE_SPREAD, s);
             const int nw = p->opts.no_floating_mean ? 0 : 1;
+            if (p->list_tiles) {                            // cuFFT path: zeros into the empty tiles, occupied tiles listed
+                if (per) LS_TRY(lsb::launch_zero_list(p, ps.C, 0, (1 + nw) * ps.C, ps.C, ps.s0 == 0, s));
+                else if (ps.s0 == 0) LS_TRY(lsb::launch_zero_list(p, 1, 0, nw + ps.C, 1, 1, s));
+                else LS_TRY(lsb::launch_zero_list(p, 0, 0, ps.C, 1 + nw, 0, s));
+                ++own;
+            }
             if (per) {
                 // slots [0, C): w2_s ; slots [C, 3C): (w_s, h_s) pairs — fixed mean: [C, 2C): h_s (the rows kernel then
                 // stores the h rows only)

@@ -113,6 +113,8 @@ struct ls_plan_s {
     // own FFT (ls_fft.cu): n = 2^20 .. 2^24, fp64; opts.fft_impl
     bool own_fft = false;
     bool fft_prune = false;                         // spreading skips empty tiles, FFT pass 1 prunes by liveness masks
+    bool list_tiles = false;                        // cuFFT path: empty tiles zero-filled by a sweep kernel, spreading walks
+                                                    // the list of occupied tiles (ls_tile_zero_list_kernel)
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
     bool fuse_pass23 = false;                      // FFT passes 2 + 3 as one persistent kernel (intermediate in L2)
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
@@ -154,6 +156,7 @@ cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2,
                           int slot0_x1, cudaStream_t s);
 int spread_rows_per_group(const ls_plan_s* p);
 cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s);
+cudaError_t launch_zero_list(ls_plan_s* p, int nrows_x2, int slot0_x2, int nrows_x1, int slot0_x1, int build_list, cudaStream_t s);
 // ---- ls_fft.cu: own three-pass FFT (n = 2^20 .. 2^24, fp64) ------------------------------------------
 bool own_fft_supported(const ls_plan_s* p);
 bool own_fft_prunes(const ls_plan_s* p);          // first pass pruned by liveness masks (n >= 2^20)

@@ -238,6 +238,31 @@ def test_cfg5_scaled_fp32_clustered():
     assert e["median"] <= 1e-4, e
 
 
+def test_zero_fill_sweep_and_tile_lists_on_the_cufft_path():
+    """cuFFT path with the sweep kernel that zero-fills empty tiles and lists occupied ones (what config 5 runs at full
+    size), forced at small sizes (opts.reserved[0] = 2): fp32 clustered, fp64 non-power-of-two grid, a batch in passes,
+    per-series dy, a grid so small that every tile wraps; replays must agree (the lists are rebuilt per execute)."""
+    w = scaled_workload(5, 100_000)
+    ks = compare_indices(w, 1024)
+    Pg = gpu_power(w, reserved=(2, 0), side_stream=True, repeat=2)
+    e = errors(Pg[0][ks], oracle_power(w, ks=ks))
+    assert e["Einf"] <= GATE_F32, e
+    w2 = scaled_workload(2, 3000)
+    _check64(errors(gpu_power(w2, fft_impl=1, upsampfac=1.5, reserved=(2, 0))[0], oracle_power(w2, fast=True)), pointwise=False)
+    wb = scaled_workload(4, 1500, batch=7)
+    P_ref = gpu_power(wb, fft_impl=1, reserved=(1, 0))
+    for chunk in (0, 3):
+        assert np.max(np.abs(gpu_power(wb, fft_impl=1, reserved=(2, 0), batch_chunk=chunk) - P_ref)) <= 1e-12
+    wb.dy = np.ascontiguousarray(np.random.default_rng(3).uniform(0.5, 1.5, (7, wb.Nd)))
+    Pp = gpu_power(wb, fft_impl=1, reserved=(2, 0), batch_chunk=2)
+    for b in (0, 6):
+        _check64(errors(Pp[b], oracle_power(wb, b)))
+    rng = np.random.default_rng(8)
+    t = rng.uniform(-50.0, 150.0, 400); y = rng.normal(0, 1, 400); dy = rng.uniform(0.5, 1.5, 400)
+    ww = _custom(t, y, dy, f0=0.05, df=0.0131, Nf=700)
+    _check64(errors(gpu_power(ww, fft_impl=1, reserved=(2, 0))[0], oracle_power(ww)), pointwise=False)
+
+
 def test_cfg5_full_size_fp32_sampled_frequencies():
     w = make_workload(5)
     Pg = gpu_power(w)
