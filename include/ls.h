@@ -20,7 +20,8 @@
  * tile-owner spread, deconvolve + assemble).  The fine-grid FFT is the library's own three-pass
  * transform for fp64 power-of-two grids of 2^12..2^24 cells (first pass pruned from 2^20 cells on)
  * and one cuFFT plan for every other grid.  There is NO CPU fallback: every entry point
- * fails with LS_ERR_CUDA when no device is usable.
+ * fails with LS_ERR_CUDA when no device is usable.  From 2^20 cells on, passes 2 + 3 of the own FFT are one
+ * persistent kernel that moves its tiles with TMA (cp.async.bulk.tensor / cp.async.bulk + mbarriers).
  *
  * Conventions
  *   - All functions return an int status (LS_OK == 0); nothing throws, prints or exits.
@@ -117,7 +118,10 @@ typedef struct {
     int normalization;      /* LS_NORM_STANDARD (default), _MODEL, _LOG, _PSD            */
     int t_is_dtype;         /* 0: t is double[Nd] (default, recommended: A9).  1 with LS_F32: t is float[Nd]; it is
                                promoted exactly to double on the device before anything else reads it  */
-    int reserved[2];        /* must be zero                                                       */
+    int reserved[2];        /* zero in production.  Kernel variants kept for comparison and test knobs:
+                               reserved[0] = 1: round-1 kernels (per-thread-load FFT passes 2 + 3; one spreading CTA per
+                               tile on the cuFFT path), 2: three consumer groups in the FFT kernel / the zero-fill
+                               sweep forced on the cuFFT path; reserved[1] = queue lag of the fused FFT passes (1..8) */
 } ls_opts;
 
 /* ls_plan — choose (sigma, w, beta, n) from eps ("width and fine grid size are

@@ -110,7 +110,7 @@ struct ls_plan_s {
     size_t total_bytes = 0;
     size_t grids_bytes = 0, modes_bytes = 0;
     bool external_ws = false;   // grids / modes / fft_work live in caller memory (ls_set_workspace)
-    // own FFT (ls_fft.cu): n = 2^20 .. 2^24, fp64; opts.fft_impl
+    // own FFT (ls_fft.cu): fp64, n = 2^12 .. 2^24 (first pass pruned from 2^20 on); opts.fft_impl
     bool own_fft = false;
     bool fft_prune = false;                         // spreading skips empty tiles, FFT pass 1 prunes by liveness masks
     bool list_tiles = false;                        // cuFFT path: empty tiles zero-filled by a sweep kernel, spreading walks
@@ -157,7 +157,7 @@ cudaError_t launch_spread(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2,
 int spread_rows_per_group(const ls_plan_s* p);
 cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_zero_list(ls_plan_s* p, int nrows_x2, int slot0_x2, int nrows_x1, int slot0_x1, int build_list, cudaStream_t s);
-// ---- ls_fft.cu: own three-pass FFT (n = 2^20 .. 2^24, fp64) ------------------------------------------
+// ---- ls_fft.cu: own FFT (fp64, n = 2^12 .. 2^24; first pass pruned and passes 2 + 3 fused from 2^20 on) ------
 bool own_fft_supported(const ls_plan_s* p);
 bool own_fft_prunes(const ls_plan_s* p);          // first pass pruned by liveness masks (n >= 2^20)
 int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 (where that pass is the 16 x RB kernel)
