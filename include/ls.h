@@ -148,7 +148,11 @@ int ls_execute(ls_plan_t plan, const void* t, const void* y, const void* dy, voi
 
 /* ls_execute_host — the same with HOST buffers: copies t, y, dy to plan-owned device staging
  * buffers, executes, copies power back and synchronises the stream before returning.  Pinned
- * host memory makes the copies asynchronous with respect to each other, pageable memory works. */
+ * host memory makes the copies asynchronous with respect to each other, pageable memory works.
+ * Outputs of 8 MB and more leave the device piece by piece on a plan-owned second stream while the
+ * next piece is computed: a batch pass by pass (so a batch_chunk below the batch size hides the
+ * kernels behind the copy-out; one pass cannot), one long series (Nf >= 2^22) in frequency
+ * quarters of the assembly.  `power` is complete, and both streams idle, when the call returns. */
 int ls_execute_host(ls_plan_t plan, const void* t, const void* y, const void* dy, void* power,
                     void* cuda_stream);
 

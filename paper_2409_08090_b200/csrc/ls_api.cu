@@ -345,6 +345,8 @@ int ls_destroy(ls_plan_t p) {
     dfree(p, p->st_y);
     dfree(p, p->st_dy);
     dfree(p, p->st_p);
+    if (p->copy_stream) cudaStreamDestroy(p->copy_stream);
+    if (p->copy_ev) cudaEventDestroy(p->copy_ev);
     for (auto& ev : p->events) {
         cudaEventDestroy(ev.beg);
         cudaEventDestroy(ev.end);
@@ -595,7 +597,12 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
 }
 
 // Enqueue the whole stage sequence on stream s (directly, or into a stream capture).
-static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, cudaStream_t s) {
+//
+// host_power != nullptr (ls_execute_host, direct launches only): every finished piece of `power` — a pass's series, or
+// with a single pass a quarter of the frequencies — is copied to the host on p->copy_stream while the kernels of the
+// next piece run; the caller joins copy_stream.
+static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void* dy, void* power, cudaStream_t s,
+                           char* host_power = nullptr) {
     const bool per = p->opts.dy_per_series != 0;
     int own = 0, ffts = 0;
     cudaError_t ce = cudaSuccess;
@@ -700,10 +707,29 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
             }
 
             stage_begin(p, LS_STAGE_ASSEMBLE, s);
-            if (p->fuse_assemble)
+            const size_t RB = real_bytes(p->dtype);
+            auto copy_out = [&](size_t off, size_t bytes) -> cudaError_t {      // power[off, off + bytes) is final on s
+                cudaError_t e = cudaEventRecord(p->copy_ev, s);
+                if (e == cudaSuccess) e = cudaStreamWaitEvent(p->copy_stream, p->copy_ev, 0);
+                if (e == cudaSuccess) e = cudaMemcpyAsync(host_power + off, (const char*)power + off, bytes, cudaMemcpyDeviceToHost, p->copy_stream);
+                return e;
+            };
+            if (p->fuse_assemble) {
                 LS_TRY(lsb::launch_own_fft_assemble(p, h_slot, ps.C, ps.s0, w_slot, w2_slot, power, s));
-            else
+                if (host_power) LS_TRY(copy_out((size_t)ps.s0 * p->Nf * RB, (size_t)ps.C * p->Nf * RB));
+            } else if (host_power && passes.size() == 1 && p->batch == 1 && p->Nf >= (1 << 22)) {
+                constexpr int kPieces = 4;                                       // one long series: frequency quarters
+                const long long step = ((p->Nf + kPieces - 1) / kPieces + 255) & ~255LL;
+                for (long long k0 = 0; k0 < p->Nf; k0 += step) {
+                    const long long k1 = std::min<long long>(p->Nf, k0 + step);
+                    LS_TRY(lsb::launch_assemble(p, ps.s0, ps.C, h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride, power, s, k0, k1));
+                    LS_TRY(copy_out((size_t)k0 * RB, (size_t)(k1 - k0) * RB));
+                    if (k0) ++own;
+                }
+            } else {
                 LS_TRY(lsb::launch_assemble(p, ps.s0, ps.C, h_slot, h_stride, w_slot, w_stride, w2_slot, w2_stride, power, s));
+                if (host_power) LS_TRY(copy_out((size_t)ps.s0 * p->Nf * RB, (size_t)ps.C * p->Nf * RB));
+            }
             ++own;
             stage_end(p, s);
         }
@@ -776,9 +802,28 @@ int ls_execute_host(ls_plan_t p, const void* t, const void* y, const void* dy, v
         cudaGetLastError();
         return LS_ERR_CUDA;
     }
-    const int rc = ls_execute(p, p->st_t, p->st_y, p->st_dy, p->st_p, cuda_stream);
-    if (rc != LS_OK) return rc;
-    if (cudaMemcpyAsync(power, p->st_p, bp, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+    if (bp < ((size_t)8 << 20)) {                     // small output: launch-latency-bound, one graph replay and one copy
+        const int rc = ls_execute(p, p->st_t, p->st_y, p->st_dy, p->st_p, cuda_stream);
+        if (rc != LS_OK) return rc;
+        if (cudaMemcpyAsync(power, p->st_p, bp, cudaMemcpyDeviceToHost, s) != cudaSuccess || cudaStreamSynchronize(s) != cudaSuccess) {
+            cudaGetLastError();
+            return LS_ERR_CUDA;
+        }
+        return LS_OK;
+    }
+    // Direct launches (their host cost hides behind the input copies), the power copied out piece by piece on a second
+    // stream while the next piece is computed; the stream s is joined with it before the final synchronise.
+    if (!p->copy_stream && (cudaStreamCreateWithFlags(&p->copy_stream, cudaStreamNonBlocking) != cudaSuccess ||
+                            cudaEventCreateWithFlags(&p->copy_ev, cudaEventDisableTiming) != cudaSuccess)) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    const int rc = enqueue_execute(p, p->st_t, p->st_y, p->st_dy, p->st_p, s, (char*)power);
+    if (rc != LS_OK) {
+        cudaStreamSynchronize(p->copy_stream);
+        return rc;
+    }
+    if (cudaEventRecord(p->copy_ev, p->copy_stream) != cudaSuccess || cudaStreamWaitEvent(s, p->copy_ev, 0) != cudaSuccess ||
         cudaStreamSynchronize(s) != cudaSuccess) {
         cudaGetLastError();
         return LS_ERR_CUDA;

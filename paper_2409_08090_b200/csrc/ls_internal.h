@@ -101,6 +101,8 @@ struct ls_plan_s {
     lsb::PointSet ps[2];
     // host staging for ls_execute_host
     void *st_t = nullptr, *st_y = nullptr, *st_dy = nullptr, *st_p = nullptr;
+    cudaStream_t copy_stream = nullptr;             // ls_execute_host: device -> host copies of finished power, beside the kernels
+    cudaEvent_t copy_ev = nullptr;
     // cuFFT
     cufftHandle fft_first = 0, fft_chunk = 0, fft_rem = 0;
     bool has_first = false, has_chunk = false, has_rem = false;
@@ -172,7 +174,8 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
 // ---- ls_post.cu: P0 table, K5+K6 -----------------------------------------------------------
 cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double* weights, cudaStream_t s);
 cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,
-                            int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s);
+                            int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s, long long k0 = 0,
+                            long long k1 = -1);      // frequencies [k0, k1); k1 < 0: to Nf
 cudaError_t launch_debug_modes(ls_plan_s* p, int h_slot, int w_slot, int w2_slot, int64_t K,
                                const int64_t* d_kidx, double* d_out, cudaStream_t s);
 cudaError_t launch_debug_assemble(int64_t K, const double* d_sums, double YY, double W, int no_float, int norm,

@@ -45,6 +45,7 @@ struct V2<float> { using type = float2; };
 struct AssembleArgs {
     const void* grids;              // fine grids after the FFT, or (compact) the own FFT's [slots][Nf] mode array
     long long n, Nf;
+    long long k0, k1;               // frequencies [k0, k1) of this launch
     long long stride;               // elements between transforms: n, or Nf when compact
     int compact;                    // 1: mode k of a transform sits at index k
     int no_float;                   // opts.no_floating_mean: the (S, C) sums of the weights drop out
@@ -61,8 +62,8 @@ template <typename T>
 __global__ void __launch_bounds__(kPostThreads)
 ls_assemble_kernel(const AssembleArgs a) {
     using T2 = typename V2<T>::type;
-    const long long k = (long long)blockIdx.x * kPostThreads + threadIdx.x;
-    if (k >= a.Nf) return;
+    const long long k = a.k0 + (long long)blockIdx.x * kPostThreads + threadIdx.x;
+    if (k >= a.k1) return;
     const int i = blockIdx.y;                      // series within this pass
     const int s = a.series0 + i;
     const long long kp = k - a.half;               // centred mode k'
@@ -86,8 +87,8 @@ template <typename T>
 __global__ void __launch_bounds__(kPostThreads)
 ls_assemble_shared_kernel(const AssembleArgs a, int nseries) {
     using T2 = typename V2<T>::type;
-    const long long k = (long long)blockIdx.x * kPostThreads + threadIdx.x;
-    if (k >= a.Nf) return;
+    const long long k = a.k0 + (long long)blockIdx.x * kPostThreads + threadIdx.x;
+    if (k >= a.k1) return;
     const long long kp = k - a.half;
     const long long idx = a.compact ? k : (kp < 0 ? kp + a.n : kp);
     const double d = a.dinv[kp < 0 ? -kp : kp];
@@ -154,8 +155,10 @@ cudaError_t launch_deconv_table(ls_plan_s* p, const double* nodes, const double*
 }
 
 cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, int h_stride, int w_slot,
-                            int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s) {
+                            int w_stride, int w2_slot, int w2_stride, void* power, cudaStream_t s, long long k0, long long k1) {
     AssembleArgs a;
+    a.k0 = k0;
+    a.k1 = k1 < 0 ? p->Nf : k1;
     a.grids = p->own_fft ? p->modes : p->grids;
     a.n = p->n;
     a.Nf = p->Nf;
@@ -172,7 +175,7 @@ cudaError_t launch_assemble(ls_plan_s* p, int series0, int nseries, int h_slot, 
     a.w_slot = w_slot; a.w_stride = w_stride;
     a.w2_slot = w2_slot; a.w2_stride = w2_stride;
     a.power = power;
-    const unsigned gx = (unsigned)((p->Nf + kPostThreads - 1) / kPostThreads);
+    const unsigned gx = (unsigned)((a.k1 - a.k0 + kPostThreads - 1) / kPostThreads);
     if (nseries > 1 && h_stride == 1 && w_stride == 0 && w2_stride == 0) {       // shared dy
         dim3 grid(gx, (nseries + kSeriesPerThread - 1) / kSeriesPerThread);
         if (p->dtype == LS_F64) ls_assemble_shared_kernel<double><<<grid, kPostThreads, 0, s>>>(a, nseries);

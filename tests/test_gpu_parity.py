@@ -398,6 +398,25 @@ def test_execute_host_matches_device():
     assert np.max(np.abs(gpu_power(w5) - gpu_power(w5, host=True))) <= 1e-5
 
 
+def test_execute_host_overlapped_copy_out():
+    """Outputs of >= 8 MB leave the device piece by piece on a second stream while the next piece is computed
+    (ls.h, ls_execute_host): a long single series in frequency quarters (own FFT), and a batch pass by pass
+    (shared and per-series dy, batch_chunk forcing several passes with a ragged last one).  The kernels are the
+    device path's: same numbers — bit for bit where no atomics' order is involved in the sums."""
+    w = scaled_workload(3, 400_000)                     # Nf = 5e6: four assembly launches of 1.25e6 frequencies
+    assert w.Nf * 8 >= 8 << 20 and w.Nf >= 1 << 22
+    Pd, Ph = gpu_power(w), gpu_power(w, host=True)
+    assert np.all(np.isfinite(Ph)) and np.max(np.abs(Pd - Ph)) <= 1e-11
+    wb = scaled_workload(4, 4000, batch=23)             # 23 x 50 000 x 8 B = 9.2 MB
+    assert wb.batch * wb.Nf * 8 >= 8 << 20
+    Pd = gpu_power(wb, batch_chunk=5)
+    Ph = gpu_power(wb, host=True, batch_chunk=5)        # 5 passes, the last of 3 series
+    assert np.all(np.isfinite(Ph)) and np.max(np.abs(Pd - Ph)) <= 1e-11
+    rng = np.random.default_rng(3)
+    wp = Workload(wb.name, wb.t, wb.y, rng.uniform(0.5, 1.5, wb.y.shape), wb.f0, wb.df, wb.Nf, "f64", wb.eps)
+    assert np.max(np.abs(gpu_power(wp, batch_chunk=7) - gpu_power(wp, host=True, batch_chunk=7))) <= 1e-11
+
+
 def test_graph_replay_matches_direct_launches():
     """opts.graph = 2 on a side stream: capture once, replay, re-capture when a buffer changes; identical
     to direct launches (graph = 1)."""
