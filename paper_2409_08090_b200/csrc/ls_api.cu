@@ -332,6 +332,7 @@ int ls_destroy(ls_plan_t p) {
     dfree(p, p->t64);
     dfree(p, p->fft_wlo);
     dfree(p, p->fft_whi);
+    dfree(p, p->ftab);
     dfree(p, p->tile_list);
     dfree(p, p->zeroed);                     // sums and both histograms live in this allocation
     dfree(p, p->scan_tmp);
@@ -398,6 +399,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     // [1.25 Nf, 2.5 Nf) (the FFT pass count, not the cell count, decides its time), the
     // width follows from the realised sigma = n/Nf, plus two (fp64) / one (fp32) cells of safety so
     // that a pointwise reading of the tolerance also holds (A8, A9).
+    bool auto5 = false;                                 // the plan chose a 5 x 2^k grid for the own fused transform
     if (o.upsampfac != 0.0) {
         const double want = ceil(o.upsampfac * (double)Nf);
         if (want >= 2147483000.0) { delete p; return LS_ERR_UNSUPPORTED; }
@@ -409,6 +411,16 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         while ((double)m < want) m *= 2;
         p->n = m;
         const int ntrans = (o.dy_per_series ? 3 * batch : batch + 2) - (o.no_floating_mean ? (o.dy_per_series ? batch : 1) : 0);
+        // A batch of small fp64 grids with shared dy: where 5 x 2^k (k = 13 .. 16) lies between 1.25 Nf and the power of two,
+        // the own two-pass transform on it with the assembly fused into the last pass moves the fewest bytes (config 4:
+        // 163 840 cells instead of 2^18, or of cuFFT on 160 000: 3.17 -> 2.72 ms per 1000 series).
+        int64_t n5 = 0;
+        for (int k = 13; k <= 16; ++k)
+            if ((double)(5LL << k) >= want && (5LL << k) < m) n5 = n5 ? n5 : (5LL << k);
+        if (n5 && dtype == LS_F64 && !o.dy_per_series && o.fft_impl != 1 && !o.no_autotune && (double)n5 * ntrans * 16.0 > 64e6) {
+            p->n = n5;
+            auto5 = true;
+        } else
         if ((double)m > 1.6 * (double)Nf && (double)m * ntrans >= (double)((int64_t)1 << 20) && !o.no_autotune) {
             // the timed choice is cached per (Nf, dtype, transforms, device): the same arguments give the same grid — and
             // therefore the same results — for the life of the process (between processes it may differ: ls.h)
@@ -477,7 +489,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     // them, for problems small enough to be latency-bound (cuFFT runs a 2^14-point fp64 transform in ONE CTA: 29 us of
     // config 1's 58), but not for large batches of small grids, where cuFFT's pass structure moves fewer bytes
     p->own_fft = o.fft_impl != 1 && lsb::own_fft_supported(p);
-    if (p->own_fft && o.fft_impl == 0 && !lsb::own_fft_prunes(p) && (double)p->M * (double)p->n * 16.0 > 64e6) p->own_fft = false;
+    if (p->own_fft && o.fft_impl == 0 && !auto5 && !lsb::own_fft_prunes(p) && (double)p->M * (double)p->n * 16.0 > 64e6) p->own_fft = false;
     p->fft_prune = p->own_fft && lsb::own_fft_prunes(p);
     // cuFFT path, few transforms over very many tiles (config 5: 3 x 154 000): one sweep kernel zero-fills the empty tiles
     // and lists the occupied ones for a persistent spreading launch.  Measured: config 5 spread 1.51 -> 1.34 ms; config 4
@@ -488,10 +500,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     // Measured at config 3 (profiles/r1e_cfg3.md): with the cheaper assembly arithmetic the separate
     // assembly kernel (0.118 ms at 81 % of DRAM peak) plus an unfused third pass beats the fused kernel, which is
     // bound by its 2-CTAs-per-SM arithmetic, by 1 % — so fusion is opt-in (fft_impl = 2), not the default.
-    p->fuse_assemble = p->own_fft && o.fft_impl == 2 && !o.dy_per_series;
+    p->fuse_assemble = p->own_fft && (o.fft_impl == 2 || (auto5 && o.fft_impl == 0)) && !o.dy_per_series;
     // Passes 2 and 3 as one persistent kernel with the intermediate kept in L2 (ls_fft.cu): the default wherever
     // the pruned three-pass transform runs; fft_impl = 3 keeps the three separate launches (for comparison).
-    p->fuse_pass23 = p->fft_prune && !p->fuse_assemble && o.fft_impl != 3;
+    p->fuse_pass23 = p->fft_prune && !lsb::own_fft_rm5(p) && !p->fuse_assemble && o.fft_impl != 3;
 
     // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
     p->ndf = two_prod((double)p->n, df);
@@ -514,13 +526,14 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
             if ((ce = dmalloc(p, (char**)&p->fft_whi, (size_t)std::max<int64_t>(4096, p->n / 4096) * 16)) != cudaSuccess) break;
             p->modes_bytes = (size_t)p->slots * Nf * 16;
             if ((ce = dmalloc(p, (char**)&p->modes, p->modes_bytes)) != cudaSuccess) break;
+            if (p->fuse_assemble && (ce = dmalloc(p, (char**)&p->ftab, (size_t)Nf * 32)) != cudaSuccess) break;
             if ((ce = lsb::own_fft_init(p, 0)) != cudaSuccess) break;
         }
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
         const size_t mask_bytes = p->fft_prune ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : (p->list_tiles ? 256 : 0);   // masks + 2 list counters
-        const size_t queue_bytes = p->fft_prune ? (((size_t)(2 + 32 * p->slots) * 4 + 255) & ~(size_t)255) : 0;
+        const size_t queue_bytes = p->fuse_pass23 ? (((size_t)(2 + 32 * p->slots) * 4 + 255) & ~(size_t)255) : 0;
         p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes + queue_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;
         if (queue_bytes) p->fft_queue = (int*)((char*)p->zeroed + sums_bytes + hist_bytes + mask_bytes);
@@ -690,7 +703,7 @@ static int enqueue_execute(ls_plan_t p, const void* t, const void* y, const void
                 stage_begin(p, LS_STAGE_FFT_PASS3, s);
                 LS_TRY(lsb::launch_own_fft_pass3(p, ps.fft_slot0, n_modes, s));
                 stage_end(p, s);
-                own += 1 + (p->n > 65536 ? 1 : 0) + (n_modes > 0 ? 1 : 0);
+                own += 1 + ((p->n > 65536 && !lsb::own_fft_rm5(p)) ? 1 : 0) + (n_modes > 0 ? 1 : 0);
                 }
             } else {
                 stage_begin(p, LS_STAGE_FFT, s);

@@ -124,6 +124,8 @@ struct FftArgs {
     // series0 + i; the (w, w2) modes are read from the compact array
     const double2* w_modes;    // [Nf] modes of w at x1
     const double2* w2_modes;   // [Nf] modes of w at x2
+    int series_major;          // fused batch launch: grid = (series, tiles)
+    const double2* ftab;       // [Nf][2] per-frequency terms of the fused assembly: (d Cw, d Sw), (1/CC, 1/SS)
     const double* dinv;        // 1 / psihat(|k'|)
     const double* sums;        // [batch][4]: YY at [4 s + 2]
     double* power;             // [batch][Nf]
@@ -308,6 +310,102 @@ ls_fft_pass1_small_kernel(const FftArgs a, long long inner) {
     }
 }
 
+// First pass for n = 5 * 2^k cells, two passes R1 x 256 with R1 = 80 RM rows (RM = 2, 4, 8, 16: n = 40 960 .. 327 680):
+// the sizes that sit halfway between the powers of two (sigma = n / Nf in [1.25, 1.77) where the power of two has
+// [1.77, 2.5): a batch of small grids moves 1.6 x fewer bytes).  R1 = 16 x RM x 5, decimation in frequency, J = 5 RM:
+//   l1 = J i + j,  j = 5 p + q          (i < 16, p < RM, q < 5)
+//   k1 = ka + 16 (kp + RM kq)           (ka < 16, kp < RM, kq < 5)
+//   stage 1: 16-point FFTs over i -> ka, times w_R1^{ka j};      one per thread (J threads per column)
+//   stage 2: RM-point FFTs over p -> kp, times w_R1^{16 kp q};   80 per column
+//   stage 3: 5-point FFTs over q -> kq, times the inter-pass twiddle w_n^{k1 m};  16 RM per column
+// The column tile (R1 rows x 8 columns) lives in shared memory between the stages ([ka][j][c], 128-byte rows: every
+// access of a quarter warp is one row, conflict-free); 128-byte global segments on both sides, in place.
+constexpr int kC5 = 8;                   // columns per CTA
+constexpr double kCos5a = 0.30901699437494742410;    // cos(2 pi / 5)
+constexpr double kCos5b = -0.80901699437494742410;   // cos(4 pi / 5)
+constexpr double kSin5a = 0.95105651629515357212;    // sin(2 pi / 5)
+constexpr double kSin5b = 0.58778525229247312917;    // sin(4 pi / 5)
+// X_k = sum_l x_l e^{+2 pi i k l / 5}, in place, natural order
+__device__ __forceinline__ void fft5(double2 (&x)[5]) {
+    const double2 t1 = cadd(x[1], x[4]), t2 = cadd(x[2], x[3]), t3 = csub(x[1], x[4]), t4 = csub(x[2], x[3]);
+    const double2 a1 = make_double2(x[0].x + kCos5a * t1.x + kCos5b * t2.x, x[0].y + kCos5a * t1.y + kCos5b * t2.y);
+    const double2 a2 = make_double2(x[0].x + kCos5b * t1.x + kCos5a * t2.x, x[0].y + kCos5b * t1.y + kCos5a * t2.y);
+    const double2 b1 = make_double2(kSin5a * t3.x + kSin5b * t4.x, kSin5a * t3.y + kSin5b * t4.y);
+    const double2 b2 = make_double2(kSin5b * t3.x - kSin5a * t4.x, kSin5b * t3.y - kSin5a * t4.y);
+    x[0] = make_double2(x[0].x + t1.x + t2.x, x[0].y + t1.y + t2.y);
+    x[1] = make_double2(a1.x - b1.y, a1.y + b1.x);      // a1 + i b1
+    x[4] = make_double2(a1.x + b1.y, a1.y - b1.x);      // a1 - i b1
+    x[2] = make_double2(a2.x - b2.y, a2.y + b2.x);
+    x[3] = make_double2(a2.x + b2.y, a2.y - b2.x);
+}
+template <int RM>
+constexpr size_t cols5_smem() { return sizeof(double2) * (size_t)(80 * RM) * (kC5 + 1); }   // tile + w_R1 table
+template <int RM>
+__global__ void __launch_bounds__(5 * RM * kC5, 16 / RM)      // 640 threads per SM: two CTAs at RM = 8 need <= 102 registers
+ls_fft_cols5_kernel(const FftArgs a) {
+    constexpr int J = 5 * RM, R1 = 16 * J;
+    extern __shared__ __align__(16) unsigned char fsm[];
+    double2* S = reinterpret_cast<double2*>(fsm);            // [ka][j][c]
+    double2* wr = S + R1 * kC5;                              // w_R1^x, x < R1
+    for (int x = threadIdx.x; x < R1; x += J * kC5) {
+        double sn, cs;
+        sincospi(2.0 * (double)x / (double)R1, &sn, &cs);
+        wr[x] = make_double2(cs, sn);
+    }
+    const int c = threadIdx.x % kC5, tj = threadIdx.x / kC5;
+    const int m = blockIdx.x * kC5 + c, tr = blockIdx.y;
+    double2* base = a.grids + (long long)tr * a.n + m;
+    {
+        const int j = tj;
+        double2 x[16];
+        // rows of tiles the spreading kernel never wrote are zeros that are not in memory: one liveness bit per tile
+        const unsigned* masks = a.row_masks ? a.row_masks + (tr < a.set_of_trans_first ? 0 : 32) : nullptr;
+        const int rshift = a.tile_shift - 8;                 // rows (256 cells) per spreading tile, log2
+#pragma unroll
+        for (int i = 0; i < 16; ++i) {
+            const int row = J * i + j, tile = row >> rshift;
+            x[i] = make_double2(0.0, 0.0);
+            if (!masks || ((__ldg(&masks[tile & 31]) >> (tile >> 5)) & 1u)) x[i] = base[(long long)row * 256];
+        }
+        fft16(x);
+        __syncthreads();                                     // table ready
+#pragma unroll
+        for (int ka = 0; ka < 16; ++ka) S[(ka * J + j) * kC5 + c] = cmul(x[pos16(ka)], wr[ka * j]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 80 / J; ++r) {                       // stage 2: butterfly (ka, q), elements S[ka][5 p + q]
+        const int b = tj + J * r, ka = b & 15, q = b >> 4;
+        double2 y[RM];
+#pragma unroll
+        for (int p = 0; p < RM; ++p) y[p] = S[(ka * J + 5 * p + q) * kC5 + c];
+        fft_small<RM>(y);
+#pragma unroll
+        for (int kp = 0; kp < RM; ++kp) S[(ka * J + 5 * kp + q) * kC5 + c] = cmul(y[fft_pos<RM>(kp)], wr[16 * kp * q]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int r = 0; r < 4; ++r) {                            // stage 3: butterfly (ka, kp), elements S[ka][5 kp + q]
+        const int b = tj + J * r;
+        if (b < 16 * RM) {
+            const int ka = b & 15, kp = b >> 4;
+            double2 z[5];
+#pragma unroll
+            for (int q = 0; q < 5; ++q) z[q] = S[(ka * J + 5 * kp + q) * kC5 + c];
+            fft5(z);
+            // k1 = k0 + 16 RM kq, k0 = ka + 16 kp: w_n^{k1 m} = w_n^{k0 m} (w_n^{16 RM m})^kq; both exponents < n
+            const unsigned e0 = (unsigned)(ka + 16 * kp) * (unsigned)m, es = (unsigned)(16 * RM) * (unsigned)m;
+            double2 tw = cmul(__ldg(&a.wlo[e0 & 4095u]), __ldg(&a.whi[e0 >> 12]));
+            const double2 st = cmul(__ldg(&a.wlo[es & 4095u]), __ldg(&a.whi[es >> 12]));
+#pragma unroll
+            for (int kq = 0; kq < 5; ++kq) {
+                base[(long long)(ka + 16 * (kp + RM * kq)) * 256] = cmul(z[kq], tw);
+                tw = cmul(tw, st);
+            }
+        }
+    }
+}
+
 // Pass 3: the transform dimension (l3) is contiguous; the CTA takes 16 consecutive k1 at one k2, so that the
 // kept modes leave in runs of 16 consecutive frequencies.  Output: modes[tr][k], k = (kk + half) mod n < Nf,
 // kk = k1 + R1 k2 + R1 R2 k3 the stored mode index (= k' mod n).
@@ -321,12 +419,15 @@ ls_fft_rows_kernel(const FftArgs a) {
     double2* w256 = Y + 256 * (kC + 1);
     fill_w256(w256);
     // rows are numbered rho = k1 + R1 k2 (the low part of the output index): 16 consecutive rho per CTA
-    const int rho_b = blockIdx.x * kC, tr = blockIdx.z;
+    // series_major (fused batch): consecutive CTAs are the SAME tile of consecutive series, so that the tile's table entries
+    // (ls_freq_table_kernel) are found in L1 by all but the first CTA an SM runs on it
+    const int rho_b = (a.series_major ? blockIdx.y : blockIdx.x) * kC, tr = a.series_major ? blockIdx.x : blockIdx.z;
     const double2* src = a.grids + (long long)tr * a.n;
     double2 x[16];
     {
         const int j = threadIdx.x & 15, c = threadIdx.x >> 4;
-        const int rho = rho_b + c, k1 = rho & (a.R1 - 1), k2 = rho >> a.R1_shift;
+        const int rho = rho_b + c;
+        const int k1 = a.R2 == 1 ? rho : (rho & (a.R1 - 1)), k2 = a.R2 == 1 ? 0 : (rho >> a.R1_shift);   // two passes: R1 need not be 2^k
         const double2* row = src + ((long long)k1 * a.R2 + k2) * a.R3;
 #pragma unroll
         for (int i = 0; i < 16; ++i) x[i] = row[16 * i + j];
@@ -348,33 +449,29 @@ ls_fft_rows_kernel(const FftArgs a) {
         const double YYs = FUSED ? a.sums[4 * ser + 2] : 1.0;
         const double inv_YY = 1.0 / YYs;
         if (FUSED) {
-            // K5: diagonal rescaling of the three modes of frequency k; K6: tau rotation and power.  Four
-            // frequencies at a time: their 12 loads are in flight together before any arithmetic starts.
+            // K5 + K6 with the per-frequency part (1/psihat, the tau rotation, 1/CC, 1/SS: functions of the weights only)
+            // read from the table ls_freq_table_kernel made of the (w, w2) modes: what is left per series is the rotation
+            // of its h mode and two squares.  Four frequencies at a time: their loads are in flight together.
 #pragma unroll
             for (int g = 0; g < 16; g += 4) {
                 long long k[4];
-                double d[4];
-                double2 gw[4], g2[4];
+                double2 fr[4], fi[4];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     k[q] = kk0 + r12 * (ka + 16 * (g + q)) + a.half;
                     if (k[q] >= a.n) k[q] -= a.n;
-                    d[q] = 0.0;
-                    gw[q] = g2[q] = make_double2(0.0, 0.0);
+                    fr[q] = fi[q] = make_double2(0.0, 0.0);
                     if (k[q] < a.Nf) {
-                        const long long kp = k[q] - a.half;
-                        d[q] = __ldg(&a.dinv[kp < 0 ? -kp : kp]);
-                        gw[q] = __ldg(&a.w_modes[k[q]]);
-                        g2[q] = __ldg(&a.w2_modes[k[q]]);
+                        fr[q] = __ldg(&a.ftab[2 * k[q]]);
+                        fi[q] = __ldg(&a.ftab[2 * k[q] + 1]);
                     }
                 }
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
                     if (k[q] < a.Nf) {
-                        const double2 gh = x[pos16(g + q)];
-                        const double dw = (VARIANT && a.no_float) ? 0.0 : d[q];       // fixed mean: S = C = 0
-                        const FreqTerms f = freq_terms(gw[q].y * dw, gw[q].x * dw, g2[q].y * d[q], g2[q].x * d[q]);
-                        double P = series_power(f, gh.y * d[q], gh.x * d[q], inv_YY);
+                        const double2 gh = x[pos16(g + q)];                          // (Ch, Sh) / d
+                        const double YC = gh.x * fr[q].x + gh.y * fr[q].y, YS = gh.y * fr[q].x - gh.x * fr[q].y;
+                        double P = (YC * YC * fi[q].x + YS * YS * fi[q].y) * inv_YY;
                         if (VARIANT) P = apply_normalization(P, a.norm, YYs, a.sums[0]);
                         a.power[(long long)ser * a.Nf + k[q]] = P;
                     }
@@ -630,6 +727,84 @@ __device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigne
 }
 __device__ __forceinline__ void group_barrier(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
 
+// Last pass fused with K5 + K6 for a BATCH with shared dy (fuse_assemble, >= 8 series): the per-frequency table
+// (ls_freq_table_kernel) is the same for every series, so a CTA owns one tile position — 8 consecutive rows rho, all 256
+// k3: 2048 frequencies — stages that tile's table entries in shared memory ONCE (64 KB) and then streams series through
+// it: four groups of 128 threads, each transforming one series' tile at a time (16 points per thread, one exchange through
+// the group's own buffer, group-wide named barriers only).  The ls_fft_rows_kernel<true> form reads 32 table bytes per
+// 16 data bytes out of L2 for every series (config 4: 0.95 ms, L2-bound); this one reads them once per 32 series.
+constexpr int kRbC = 8;                  // rows per tile
+constexpr int kRbGroups = 4;
+constexpr int kRbThreads = 128 * kRbGroups;
+constexpr size_t kRbSmem = sizeof(double2) * ((size_t)2 * 256 * kRbC + 256 + (size_t)kRbGroups * 256 * (kRbC + 1));
+__global__ void __launch_bounds__(kRbThreads, 1)
+ls_fft_rows_batch_kernel(const FftArgs a, int nseries, int series_per_cta) {
+    constexpr int C = kRbC;
+    extern __shared__ __align__(16) unsigned char fsm[];
+    double2* tab = reinterpret_cast<double2*>(fsm);          // [k3][c][2]: (d Cw, d Sw), (1/CC, 1/SS); zeros where k >= Nf
+    double2* w256 = tab + 2 * 256 * C;
+    const int grp = threadIdx.x >> 7, t = threadIdx.x & 127;
+    double2* Y = w256 + 256 + grp * 256 * (C + 1);           // [ka][j][C + 1]
+    fill_w256(w256, kRbThreads);
+    const int rho_b = blockIdx.x * C;
+    const long long r12 = (long long)a.R1 * a.R2;
+    for (int e = threadIdx.x; e < 256 * C; e += kRbThreads) {
+        const int c = e % C, k3 = e / C;
+        long long k = rho_b + c + r12 * k3 + a.half;
+        if (k >= a.n) k -= a.n;
+        double2 fr = make_double2(0.0, 0.0), fi = fr;
+        if (k < a.Nf) {
+            fr = __ldg(&a.ftab[2 * k]);
+            fi = __ldg(&a.ftab[2 * k + 1]);
+        }
+        tab[2 * e] = fr;
+        tab[2 * e + 1] = fi;
+    }
+    __syncthreads();
+    const int s_end = min(nseries, ((int)blockIdx.y + 1) * series_per_cta);
+    for (int i = blockIdx.y * series_per_cta + grp; i < s_end; i += kRbGroups) {
+        const double2* src = a.grids + (long long)i * a.n;
+        double2 x[16];
+        {
+            const int j = t & 15, c = t >> 4;
+            const int rho = rho_b + c;
+            const int k1 = a.R2 == 1 ? rho : (rho & (a.R1 - 1)), k2 = a.R2 == 1 ? 0 : (rho >> a.R1_shift);
+            const double2* row = src + ((long long)k1 * a.R2 + k2) * a.R3;
+#pragma unroll
+            for (int q = 0; q < 16; ++q) x[q] = __ldcs(&row[16 * q + j]);
+            fft16(x);
+#pragma unroll
+            for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
+        }
+        group_barrier(1 + grp);
+        {
+            const int c = t % C, ka = t / C;
+#pragma unroll
+            for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * (C + 1) + c];
+            group_barrier(1 + grp);                          // Y is free for the group's next series
+            fft16(x);
+            const int ser = a.series0 + i;
+            const double YYs = a.sums[4 * ser + 2];
+            const double inv_YY = 1.0 / YYs;
+            double* out = a.power + (long long)ser * a.Nf;
+#pragma unroll
+            for (int kb = 0; kb < 16; ++kb) {
+                const int k3 = ka + 16 * kb;
+                long long k = rho_b + c + r12 * k3 + a.half;
+                if (k >= a.n) k -= a.n;
+                if (k < a.Nf) {
+                    const double2 fr = tab[2 * (k3 * C + c)], fi = tab[2 * (k3 * C + c) + 1];
+                    const double2 gh = x[pos16(kb)];                                 // (Ch, Sh) / d
+                    const double YC = gh.x * fr.x + gh.y * fr.y, YS = gh.y * fr.x - gh.x * fr.y;
+                    double P = (YC * YC * fi.x + YS * YS * fi.y) * inv_YY;
+                    if (a.norm) P = apply_normalization(P, a.norm, YYs, a.sums[0]);
+                    __stcs(&out[k], P);
+                }
+            }
+        }
+    }
+}
+
 template <int k23Groups>                                 // consumer groups (128 threads, one tile at a time each)
 __global__ void __launch_bounds__(k23threads(k23Groups), 1)
 ls_fft_pass23_tma_kernel(const FftArgs a, const __grid_constant__ CUtensorMap tmap, int row0, int nslabs, int lag,
@@ -845,6 +1020,21 @@ ls_fft_pass23_tma_kernel(const FftArgs a, const __grid_constant__ CUtensorMap tm
     }
 }
 
+// Fused assembly, shared dy: the per-frequency terms of K5 + K6 from the compact (w, w2) modes, once per execute.
+__global__ void ls_freq_table_kernel(const double2* __restrict__ w_modes, const double2* __restrict__ w2_modes,
+                                     const double* __restrict__ dinv, long long Nf, long long half, int no_float,
+                                     double2* __restrict__ ftab) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= Nf) return;
+    const long long kp = k - half;
+    const double d = dinv[kp < 0 ? -kp : kp];
+    const double2 gw = w_modes[k], g2 = w2_modes[k];
+    const double dw = no_float ? 0.0 : d;                   // fixed mean: S = C = 0
+    const FreqTerms f = freq_terms(gw.y * dw, gw.x * dw, g2.y * d, g2.x * d);
+    ftab[2 * k] = make_double2(f.Cw * d, f.Sw * d);
+    ftab[2 * k + 1] = make_double2(f.iCC, f.iSS);
+}
+
 __global__ void ls_fft_tables_kernel(double2* wlo, double2* whi, long long n) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < 4096) {
@@ -872,14 +1062,24 @@ constexpr size_t k23Smem = sizeof(double2) * (256 * (kC23 + 1) + 256);
 //                 masks (needs spreading tiles that divide a pass-1 row of 65536 cells);
 //   2^17 .. 2^19: three passes with a small first radix R1 = 2, 4, 8 (ls_fft_pass1_small_kernel), unpruned;
 //   2^12 .. 2^16: two passes R1 x 256, R1 = 16 .. 256, unpruned.
+//   5 x 2^13 .. 5 x 2^16: two passes R1 x 256, R1 = 160 .. 1280 = 16 x RM x 5 (ls_fft_cols5_kernel), unpruned.
+int own_fft_rm5(const ls_plan_s* p) {                     // RM of the 5 x 2^k sizes, else 0
+    for (int rm = 2; rm <= 16; rm *= 2)
+        if (p->n == (int64_t)80 * rm * 256) return rm;
+    return 0;
+}
 bool own_fft_supported(const ls_plan_s* p) {
     const bool pow2 = (p->n & (p->n - 1)) == 0;
+    if (p->dtype == LS_F64 && own_fft_rm5(p)) return true;
     if (p->dtype != LS_F64 || !pow2 || p->n < ((int64_t)1 << 12) || p->n > ((int64_t)1 << 24)) return false;
     return p->n < ((int64_t)1 << 20) || 65536 % p->L == 0;
 }
-bool own_fft_prunes(const ls_plan_s* p) { return p->n >= ((int64_t)1 << 20); }
+bool own_fft_prunes(const ls_plan_s* p) { return p->n >= ((int64_t)1 << 20) || own_fft_rm5(p) != 0; }
+// spreading tiles per liveness-mask column: 65536 / L where the first pass works on rows of 65536 cells; 1 at the 5 x 2^k
+// sizes (rows of 256 cells: the masks are then one bit per TILE, word = tile % 32, bit = tile / 32 — at most 1280 tiles)
+int own_fft_ncoltiles(const ls_plan_s* p) { return own_fft_rm5(p) ? 1 : std::max(1, 65536 / p->L); }
 // radix of the first pass / 16 where that pass is the 16 x RB kernel (n >= 2^20: R1 = n / 2^16; n <= 2^16: R1 = n / 2^8)
-int own_fft_rb(const ls_plan_s* p) { return (int)(p->n >= ((int64_t)1 << 20) ? p->n >> 20 : p->n >> 12); }
+int own_fft_rb(const ls_plan_s* p) { return own_fft_rm5(p) ? 32 : (int)(p->n >= ((int64_t)1 << 20) ? p->n >> 20 : p->n >> 12); }
 
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     const int cnt = (int)std::max<long long>(4096, p->n / 4096);
@@ -892,6 +1092,11 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<2, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_rows_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRbSmem)) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<2>())) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<4>())) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<8>())) != cudaSuccess) return e;
+    if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<16>())) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<kC23>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_tma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23TmaSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23TmaSmem)) != cudaSuccess) return e;
@@ -906,14 +1111,14 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.grids = (double2*)p->grids + (long long)slot0 * p->n;
     a.n = p->n;
     a.R3 = 256;
-    a.R2 = p->n > 65536 ? 256 : 1;                         // two passes up to 2^16 cells
+    a.R2 = (p->n > 65536 && !own_fft_rm5(p)) ? 256 : 1;    // two passes up to 2^16 cells and at the 5 x 2^k sizes
     a.R1 = (int)(p->n / ((long long)a.R2 * a.R3));
     a.R1_shift = 0;
     while ((1 << a.R1_shift) < a.R1) ++a.R1_shift;
     a.wlo = (const double2*)p->fft_wlo;
     a.whi = (const double2*)p->fft_whi;
     a.row_masks = own_fft_prunes(p) ? p->row_masks : nullptr;
-    a.ncoltiles = std::max(1, 65536 / p->L);
+    a.ncoltiles = own_fft_ncoltiles(p);
     a.set_of_trans_first = n_x2;
     a.tile_shift = 0;
     while ((1 << a.tile_shift) < p->L) ++a.tile_shift;
@@ -921,6 +1126,8 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.Nf = p->Nf;
     a.half = p->Nf / 2;
     a.w_modes = a.w2_modes = nullptr;
+    a.ftab = (const double2*)p->ftab;
+    a.series_major = 0;
     a.dinv = p->dinv;
     a.sums = p->sums;
     a.power = nullptr;
@@ -935,6 +1142,16 @@ cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, 
     FftArgs a;
     fill_common(p, a, slot0, n_x2);
     const long long inner1 = (long long)a.R2 * a.R3;       // 65536 (three passes) or 256 (two passes)
+    if (const int rm = own_fft_rm5(p)) {                   // n = 5 x 2^k
+        const dim3 g(256 / kC5, ntrans);
+        switch (rm) {
+            case 2: ls_fft_cols5_kernel<2><<<g, 5 * 2 * kC5, cols5_smem<2>(), s>>>(a); break;
+            case 4: ls_fft_cols5_kernel<4><<<g, 5 * 4 * kC5, cols5_smem<4>(), s>>>(a); break;
+            case 8: ls_fft_cols5_kernel<8><<<g, 5 * 8 * kC5, cols5_smem<8>(), s>>>(a); break;
+            default: ls_fft_cols5_kernel<16><<<g, 5 * 16 * kC5, cols5_smem<16>(), s>>>(a); break;
+        }
+        return cudaGetLastError();
+    }
     if (a.R1 < 16) {                                       // n = 2^17 .. 2^19
         dim3 g((unsigned)std::min<long long>((inner1 + 255) / 256, 4LL * p->num_sms), ntrans);
         if (a.R1 == 8) ls_fft_pass1_small_kernel<8><<<g, 256, 0, s>>>(a, inner1);
@@ -1034,7 +1251,27 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
     a.w2_modes = (const double2*)p->modes + (long long)w2_slot * p->Nf;
     a.power = (double*)power;
     a.series0 = series0;
+    if (series0 == 0) {                                    // first pass of the execute: the (w, w2) modes are new
+        ls_freq_table_kernel<<<(unsigned)((p->Nf + 255) / 256), 256, 0, s>>>(a.w_modes, a.w2_modes, a.dinv, a.Nf, a.half, a.no_float,
+                                                                            (double2*)p->ftab);
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+    }
+    if (p->opts.reserved[0] == 2 && nseries >= 8 && (a.R1 * a.R2) % kRbC == 0 && (a.R2 == 1 || a.R1 % kRbC == 0)) {   // a batch: table tile staged once per CTA
+        const int tiles = a.R1 * a.R2 / kRbC;
+        // series per CTA: as many as keep >= ~6 waves of CTAs on the device, at least 8 (the 64 KB table tile is then <= 1/4 of
+        // what the CTA reads), a multiple of the group count
+        int spc = std::max(8, (int)((long long)tiles * nseries / (6LL * p->num_sms)));
+        spc = std::min(64, (spc + kRbGroups - 1) / kRbGroups * kRbGroups);
+        dim3 g(tiles, (nseries + spc - 1) / spc);
+        ls_fft_rows_batch_kernel<<<g, kRbThreads, kRbSmem, s>>>(a, nseries, spc);
+        return cudaGetLastError();
+    }
     dim3 g3(a.R1 * a.R2 / kC, 1, nseries);
+    if (nseries >= 8) {
+        a.series_major = 1;
+        g3 = dim3(nseries, a.R1 * a.R2 / kC, 1);
+    }
     if (a.no_float || a.norm) ls_fft_rows_kernel<true, true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     else ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();

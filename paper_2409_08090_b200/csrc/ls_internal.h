@@ -117,6 +117,7 @@ struct ls_plan_s {
     bool fft_prune = false;                         // spreading skips empty tiles, FFT pass 1 prunes by liveness masks
     bool list_tiles = false;                        // cuFFT path: empty tiles zero-filled by a sweep kernel, spreading walks
                                                     // the list of occupied tiles (ls_tile_zero_list_kernel)
+    void* ftab = nullptr;                           // fuse_assemble: [Nf][2] double2 per-frequency assembly terms
     bool fuse_assemble = false;                    // third pass of the h transforms fused with K5 + K6
     bool fuse_pass23 = false;                      // FFT passes 2 + 3 as one persistent kernel (intermediate in L2)
     void *fft_wlo = nullptr, *fft_whi = nullptr;   // twiddle tables w_n^x, w_n^{4096 y}
@@ -161,7 +162,9 @@ cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_zero_list(ls_plan_s* p, int nrows_x2, int slot0_x2, int nrows_x1, int slot0_x1, int build_list, cudaStream_t s);
 // ---- ls_fft.cu: own FFT (fp64, n = 2^12 .. 2^24; first pass pruned and passes 2 + 3 fused from 2^20 on) ------
 bool own_fft_supported(const ls_plan_s* p);
+int own_fft_rm5(const ls_plan_s* p);              // n = 5 x 2^k (two passes 80 RM x 256): RM, else 0
 bool own_fft_prunes(const ls_plan_s* p);          // first pass pruned by liveness masks (n >= 2^20)
+int own_fft_ncoltiles(const ls_plan_s* p);        // spreading tiles per liveness-mask column
 int own_fft_rb(const ls_plan_s* p);               // pass-1 radix / 16 (where that pass is the 16 x RB kernel)
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s);
 cudaError_t own_fft_make_tmap(ls_plan_s* p);      // (re-)encode the tensor map of the fine grids (plan, ls_set_workspace)

@@ -536,7 +536,7 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
     a.tile_list = p->tile_list;
     a.w_implicit = p->opts.dy_per_series ? 0 : 1;
     a.tile_counts = p->tile_counts;
-    a.ncoltiles = std::max(1, 65536 / p->L);
+    a.ncoltiles = own_fft_ncoltiles(p);
     a.fft_rb = p->fft_prune ? own_fft_rb(p) : 1;
     a.coltile_shift = 0;
     while ((1 << a.coltile_shift) < a.ncoltiles) ++a.coltile_shift;
@@ -568,7 +568,7 @@ cudaError_t launch_t(ls_plan_s* p, int row0_x2, int nrows_x2, int slot0_x2, int 
 
 // Own-FFT path, once per execute after the bin scan: occupied-tile lists and liveness masks of both point sets.
 cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s) {
-    const int ncol = std::max(1, 65536 / p->L);
+    const int ncol = own_fft_ncoltiles(p);
     int shift = 0;
     while ((1 << shift) < ncol) ++shift;
     const int total = 2 * p->ntiles;

@@ -130,6 +130,35 @@ def test_own_fft_other_power_of_two_grids(p):
     assert int(np.argmax(P_own[0])) == kg
 
 
+@pytest.mark.parametrize("k", [13, 14, 15, 16])
+def test_own_fft_grids_of_5_times_a_power_of_two(k):
+    """n = 5 x 2^k (two passes: 80 RM x 256 with a 16 x RM x 5 first pass, RM = 2 .. 16; ls_fft_cols5_kernel), asked for
+    with upsampfac: against cuFFT on the same grid (full frequency grid, a batch of 3 with the assembly fused into the last
+    pass and as its own kernel) and against the oracle on sampled k."""
+    n = 5 << k
+    rng = np.random.default_rng(500 + k)
+    Nf = int(n / 1.3107)                                 # upsampfac 1.3108 -> ceil -> next 2,3,5-smooth even size = n
+    Nd = max(200, Nf // 12)
+    t = rng.uniform(0, 2000.0, Nd)
+    dy = rng.uniform(0.5, 1.5, Nd)
+    df = 1.0 / (5 * (t.max() - t.min()))
+    kg = Nf // 3
+    y0 = np.sin(2 * np.pi * (df + kg * df) * t + 0.4) + rng.normal(0, 1.0, Nd)
+    y = np.stack([y0, 2.0 * y0 - 1.0, y0 + np.cos(2 * np.pi * t / 11.0)])
+    w = Workload(f"n5_{k}", t, np.ascontiguousarray(y), dy, df, df, Nf, "f64", 1e-9)
+    up = n / Nf * (1 - 1e-9)
+    P_own, ex = gpu_power(w, fft_impl=2, upsampfac=up, return_plan_info=True)
+    assert ex["info"]["n"] == n and ex["launches"][1] == 0
+    P_cu, exc = gpu_power(w, fft_impl=1, upsampfac=up, return_plan_info=True)
+    assert exc["info"]["n"] == n and exc["launches"][1] == 1
+    assert np.max(np.abs(P_own - P_cu)) / P_cu.max() <= 1e-11
+    assert np.max(np.abs(gpu_power(w, fft_impl=3, upsampfac=up) - P_own)) <= 1e-13
+    ks = np.unique(np.concatenate([compare_indices(w, 200), np.arange(kg - 3, kg + 4)]))
+    for b in range(3):
+        _check64(errors(P_own[b][ks], oracle_power(w, b=b, ks=ks)))
+    assert int(np.argmax(P_own[0])) == kg
+
+
 @pytest.mark.parametrize("p,batch", [(20, 1), (21, 3), (22, 1), (23, 2)])
 def test_own_fft_fused_passes_match_separate_passes(p, batch):
     """n = 2^p >= 2^20, default plan: FFT passes 2 + 3 run as one persistent kernel whose intermediate stays in L2
