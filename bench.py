@@ -244,7 +244,9 @@ def stage_model_bytes(w, info, own_fft, L):
     rec = 4 * B                                           # one bin-sorted point record (32 B fp64 / 16 B fp32)
     rows = M * Nd * B                                     # real strengths, one row per transform
     grid = M * n * 2 * B
-    written = occupied_tile_rows(w, info, L) * L * 2 * B if own_fft else grid
+    n5 = n % 5 == 0 and (n // 5) & (n // 5 - 1) == 0
+    pruned = own_fft and (n >= 1 << 20 or n5)             # tiles without points are neither written nor read
+    written = occupied_tile_rows(w, info, L) * L * 2 * B if pruned else grid
     d = {
         "stats": 8 * Nd + batch * Nd * B + Nd * B + 2 * 4 * nbins,
         "sort": 3 * 2 * 4 * nbins,
@@ -370,7 +372,8 @@ def run_ours(args):
     if not args.upsampfac:
         popts["upsampfac"] = info["n"] / w.Nf * (1 - 1e-12) if info["n"] & (info["n"] - 1) else 0.0   # same n as `plan`
     plan_t = None
-    if popts["fft_impl"] == 2:
+    n5 = info["n"] % 5 == 0 and (info["n"] // 5) & (info["n"] // 5 - 1) == 0       # 5 x 2^k: own two-pass FFT, fused for batches
+    if popts["fft_impl"] == 2 or (popts["fft_impl"] == 0 and n5 and w.dtype == "f64"):
         try:
             plan_t = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, ldt, w.batch, timing=1, no_autotune=1,
                             **dict(popts, fft_impl=3))
@@ -466,7 +469,8 @@ def run_ours(args):
     if fused23:                                           # the library reports the fused kernel's time as pass 2
         stage["fft_pass23"] = stage.pop("fft_pass2")
         stage.pop("fft_pass3")
-    fft_stages = ["fft_pass1", "fft_pass23"] if fused23 else ["fft_pass1", "fft_pass2", "fft_pass3"]
+    two_pass = own_fft and (info["n"] <= 65536 or n5)      # R1 x 256: there is no middle pass
+    fft_stages = ["fft_pass1", "fft_pass23"] if fused23 else ["fft_pass1", "fft_pass3"] if two_pass else ["fft_pass1", "fft_pass2", "fft_pass3"]
     own_stages = ["stats", "sort", "premul", "spread", "assemble"] + (fft_stages if own_fft else [])
     dom = max(own_stages, key=lambda k: stage[k])      # the dominant OWN kernel (cuFFT, when used, is a library)
     ach = sbytes[dom] / (stage[dom] * 1e-3) / 1e9

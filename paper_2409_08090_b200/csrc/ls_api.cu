@@ -500,7 +500,9 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     // Measured at config 3 (profiles/r1e_cfg3.md): with the cheaper assembly arithmetic the separate
     // assembly kernel (0.118 ms at 81 % of DRAM peak) plus an unfused third pass beats the fused kernel, which is
     // bound by its 2-CTAs-per-SM arithmetic, by 1 % — so fusion is opt-in (fft_impl = 2), not the default.
-    p->fuse_assemble = p->own_fft && (o.fft_impl == 2 || (auto5 && o.fft_impl == 0)) && !o.dy_per_series;
+    // ... except for batches on the 5 x 2^k grids: there the modes round trip (2 x 16 bytes per frequency and series) is the
+    // largest item left and the fused pass reads its per-frequency terms from a table (config 4: 2.88 -> 2.45 ms)
+    p->fuse_assemble = p->own_fft && (o.fft_impl == 2 || (o.fft_impl == 0 && lsb::own_fft_rm5(p) && batch >= 8)) && !o.dy_per_series;
     // Passes 2 and 3 as one persistent kernel with the intermediate kept in L2 (ls_fft.cu): the default wherever
     // the pruned three-pass transform runs; fft_impl = 3 keeps the three separate launches (for comparison).
     p->fuse_pass23 = p->fft_prune && !lsb::own_fft_rm5(p) && !p->fuse_assemble && o.fft_impl != 3;

@@ -124,7 +124,6 @@ struct FftArgs {
     // series0 + i; the (w, w2) modes are read from the compact array
     const double2* w_modes;    // [Nf] modes of w at x1
     const double2* w2_modes;   // [Nf] modes of w at x2
-    int series_major;          // fused batch launch: grid = (series, tiles)
     const double2* ftab;       // [Nf][2] per-frequency terms of the fused assembly: (d Cw, d Sw), (1/CC, 1/SS)
     const double* dinv;        // 1 / psihat(|k'|)
     const double* sums;        // [batch][4]: YY at [4 s + 2]
@@ -338,6 +337,10 @@ __device__ __forceinline__ void fft5(double2 (&x)[5]) {
     x[2] = make_double2(a2.x - b2.y, a2.y + b2.x);
     x[3] = make_double2(a2.x + b2.y, a2.y - b2.x);
 }
+// Stage-2 twiddles w_{5 RM}^{kp q}: kp is unrolled and q = b >> 4 is the same for the 32 threads of a warp (b = tj + J r,
+// four consecutive tj per warp, aligned to four), so they are warp-uniform constant-bank reads — no load/store unit
+// work in a kernel that is bound by it.  [log2 RM - 1][q][kp], filled by own_fft_init.
+__constant__ double2 cTw5[4][5][16];
 template <int RM>
 constexpr size_t cols5_smem() { return sizeof(double2) * (size_t)(80 * RM) * (kC5 + 1); }   // tile + w_R1 table
 template <int RM>
@@ -381,7 +384,8 @@ ls_fft_cols5_kernel(const FftArgs a) {
         for (int p = 0; p < RM; ++p) y[p] = S[(ka * J + 5 * p + q) * kC5 + c];
         fft_small<RM>(y);
 #pragma unroll
-        for (int kp = 0; kp < RM; ++kp) S[(ka * J + 5 * kp + q) * kC5 + c] = cmul(y[fft_pos<RM>(kp)], wr[16 * kp * q]);
+        for (int kp = 0; kp < RM; ++kp)
+            S[(ka * J + 5 * kp + q) * kC5 + c] = cmul(y[fft_pos<RM>(kp)], cTw5[RM == 2 ? 0 : RM == 4 ? 1 : RM == 8 ? 2 : 3][q][kp]);
     }
     __syncthreads();
 #pragma unroll
@@ -419,9 +423,7 @@ ls_fft_rows_kernel(const FftArgs a) {
     double2* w256 = Y + 256 * (kC + 1);
     fill_w256(w256);
     // rows are numbered rho = k1 + R1 k2 (the low part of the output index): 16 consecutive rho per CTA
-    // series_major (fused batch): consecutive CTAs are the SAME tile of consecutive series, so that the tile's table entries
-    // (ls_freq_table_kernel) are found in L1 by all but the first CTA an SM runs on it
-    const int rho_b = (a.series_major ? blockIdx.y : blockIdx.x) * kC, tr = a.series_major ? blockIdx.x : blockIdx.z;
+    const int rho_b = blockIdx.x * kC, tr = blockIdx.z;
     const double2* src = a.grids + (long long)tr * a.n;
     double2 x[16];
     {
@@ -461,10 +463,9 @@ ls_fft_rows_kernel(const FftArgs a) {
                     k[q] = kk0 + r12 * (ka + 16 * (g + q)) + a.half;
                     if (k[q] >= a.n) k[q] -= a.n;
                     fr[q] = fi[q] = make_double2(0.0, 0.0);
-                    if (k[q] < a.Nf) {
-                        fr[q] = __ldg(&a.ftab[2 * k[q]]);
-                        fi[q] = __ldg(&a.ftab[2 * k[q] + 1]);
-                    }
+                    if (k[q] < a.Nf)                   // one 32-byte load per frequency
+                        asm volatile("ld.global.nc.v4.f64 {%0, %1, %2, %3}, [%4];"
+                                     : "=d"(fr[q].x), "=d"(fr[q].y), "=d"(fi[q].x), "=d"(fi[q].y) : "l"(a.ftab + 2 * k[q]));
                 }
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
@@ -726,84 +727,6 @@ __device__ __forceinline__ void bulk_load(unsigned dst, const void* src, unsigne
                  : "memory");
 }
 __device__ __forceinline__ void group_barrier(int id) { asm volatile("bar.sync %0, 128;" ::"r"(id) : "memory"); }
-
-// Last pass fused with K5 + K6 for a BATCH with shared dy (fuse_assemble, >= 8 series): the per-frequency table
-// (ls_freq_table_kernel) is the same for every series, so a CTA owns one tile position — 8 consecutive rows rho, all 256
-// k3: 2048 frequencies — stages that tile's table entries in shared memory ONCE (64 KB) and then streams series through
-// it: four groups of 128 threads, each transforming one series' tile at a time (16 points per thread, one exchange through
-// the group's own buffer, group-wide named barriers only).  The ls_fft_rows_kernel<true> form reads 32 table bytes per
-// 16 data bytes out of L2 for every series (config 4: 0.95 ms, L2-bound); this one reads them once per 32 series.
-constexpr int kRbC = 8;                  // rows per tile
-constexpr int kRbGroups = 4;
-constexpr int kRbThreads = 128 * kRbGroups;
-constexpr size_t kRbSmem = sizeof(double2) * ((size_t)2 * 256 * kRbC + 256 + (size_t)kRbGroups * 256 * (kRbC + 1));
-__global__ void __launch_bounds__(kRbThreads, 1)
-ls_fft_rows_batch_kernel(const FftArgs a, int nseries, int series_per_cta) {
-    constexpr int C = kRbC;
-    extern __shared__ __align__(16) unsigned char fsm[];
-    double2* tab = reinterpret_cast<double2*>(fsm);          // [k3][c][2]: (d Cw, d Sw), (1/CC, 1/SS); zeros where k >= Nf
-    double2* w256 = tab + 2 * 256 * C;
-    const int grp = threadIdx.x >> 7, t = threadIdx.x & 127;
-    double2* Y = w256 + 256 + grp * 256 * (C + 1);           // [ka][j][C + 1]
-    fill_w256(w256, kRbThreads);
-    const int rho_b = blockIdx.x * C;
-    const long long r12 = (long long)a.R1 * a.R2;
-    for (int e = threadIdx.x; e < 256 * C; e += kRbThreads) {
-        const int c = e % C, k3 = e / C;
-        long long k = rho_b + c + r12 * k3 + a.half;
-        if (k >= a.n) k -= a.n;
-        double2 fr = make_double2(0.0, 0.0), fi = fr;
-        if (k < a.Nf) {
-            fr = __ldg(&a.ftab[2 * k]);
-            fi = __ldg(&a.ftab[2 * k + 1]);
-        }
-        tab[2 * e] = fr;
-        tab[2 * e + 1] = fi;
-    }
-    __syncthreads();
-    const int s_end = min(nseries, ((int)blockIdx.y + 1) * series_per_cta);
-    for (int i = blockIdx.y * series_per_cta + grp; i < s_end; i += kRbGroups) {
-        const double2* src = a.grids + (long long)i * a.n;
-        double2 x[16];
-        {
-            const int j = t & 15, c = t >> 4;
-            const int rho = rho_b + c;
-            const int k1 = a.R2 == 1 ? rho : (rho & (a.R1 - 1)), k2 = a.R2 == 1 ? 0 : (rho >> a.R1_shift);
-            const double2* row = src + ((long long)k1 * a.R2 + k2) * a.R3;
-#pragma unroll
-            for (int q = 0; q < 16; ++q) x[q] = __ldcs(&row[16 * q + j]);
-            fft16(x);
-#pragma unroll
-            for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * (C + 1) + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
-        }
-        group_barrier(1 + grp);
-        {
-            const int c = t % C, ka = t / C;
-#pragma unroll
-            for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * (C + 1) + c];
-            group_barrier(1 + grp);                          // Y is free for the group's next series
-            fft16(x);
-            const int ser = a.series0 + i;
-            const double YYs = a.sums[4 * ser + 2];
-            const double inv_YY = 1.0 / YYs;
-            double* out = a.power + (long long)ser * a.Nf;
-#pragma unroll
-            for (int kb = 0; kb < 16; ++kb) {
-                const int k3 = ka + 16 * kb;
-                long long k = rho_b + c + r12 * k3 + a.half;
-                if (k >= a.n) k -= a.n;
-                if (k < a.Nf) {
-                    const double2 fr = tab[2 * (k3 * C + c)], fi = tab[2 * (k3 * C + c) + 1];
-                    const double2 gh = x[pos16(kb)];                                 // (Ch, Sh) / d
-                    const double YC = gh.x * fr.x + gh.y * fr.y, YS = gh.y * fr.x - gh.x * fr.y;
-                    double P = (YC * YC * fi.x + YS * YS * fi.y) * inv_YY;
-                    if (a.norm) P = apply_normalization(P, a.norm, YYs, a.sums[0]);
-                    __stcs(&out[k], P);
-                }
-            }
-        }
-    }
-}
 
 template <int k23Groups>                                 // consumer groups (128 threads, one tile at a time each)
 __global__ void __launch_bounds__(k23threads(k23Groups), 1)
@@ -1092,7 +1015,6 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<2, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<1, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColsSmem)) != cudaSuccess) return e;
-    if ((e = cudaFuncSetAttribute(ls_fft_rows_batch_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRbSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<2>())) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<4>())) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_cols5_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cols5_smem<8>())) != cudaSuccess) return e;
@@ -1100,6 +1022,17 @@ cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<kC23>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_tma_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23TmaSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_tma_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)k23TmaSmem)) != cudaSuccess) return e;
+    if (own_fft_rm5(p)) {
+        double2 h[4][5][16];
+        for (int v = 0; v < 4; ++v)
+            for (int q = 0; q < 5; ++q)
+                for (int kp = 0; kp < 16; ++kp) {
+                    const double ang = 2.0 * M_PI * (double)((kp * q) % (10 << v)) / (double)(10 << v);   // 5 RM = 10, 20, 40, 80
+                    h[v][q][kp] = make_double2(cos(ang), sin(ang));
+                }
+        if ((e = cudaMemcpyToSymbolAsync(cTw5, h, sizeof h, 0, cudaMemcpyHostToDevice, s)) != cudaSuccess) return e;
+        if ((e = cudaStreamSynchronize(s)) != cudaSuccess) return e;
+    }
     if ((e = own_fft_make_tmap(p)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass23_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_rows_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowsSmem)) != cudaSuccess) return e;
@@ -1127,7 +1060,6 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
     a.half = p->Nf / 2;
     a.w_modes = a.w2_modes = nullptr;
     a.ftab = (const double2*)p->ftab;
-    a.series_major = 0;
     a.dinv = p->dinv;
     a.sums = p->sums;
     a.power = nullptr;
@@ -1257,21 +1189,7 @@ cudaError_t launch_own_fft_assemble(ls_plan_s* p, int h_slot0, int nseries, int 
         cudaError_t e = cudaGetLastError();
         if (e != cudaSuccess) return e;
     }
-    if (p->opts.reserved[0] == 2 && nseries >= 8 && (a.R1 * a.R2) % kRbC == 0 && (a.R2 == 1 || a.R1 % kRbC == 0)) {   // a batch: table tile staged once per CTA
-        const int tiles = a.R1 * a.R2 / kRbC;
-        // series per CTA: as many as keep >= ~6 waves of CTAs on the device, at least 8 (the 64 KB table tile is then <= 1/4 of
-        // what the CTA reads), a multiple of the group count
-        int spc = std::max(8, (int)((long long)tiles * nseries / (6LL * p->num_sms)));
-        spc = std::min(64, (spc + kRbGroups - 1) / kRbGroups * kRbGroups);
-        dim3 g(tiles, (nseries + spc - 1) / spc);
-        ls_fft_rows_batch_kernel<<<g, kRbThreads, kRbSmem, s>>>(a, nseries, spc);
-        return cudaGetLastError();
-    }
     dim3 g3(a.R1 * a.R2 / kC, 1, nseries);
-    if (nseries >= 8) {
-        a.series_major = 1;
-        g3 = dim3(nseries, a.R1 * a.R2 / kC, 1);
-    }
     if (a.no_float || a.norm) ls_fft_rows_kernel<true, true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     else ls_fft_rows_kernel<true><<<g3, kFftThreads, kRowsSmem, s>>>(a);
     return cudaGetLastError();
