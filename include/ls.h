@@ -63,7 +63,8 @@ enum {
     LS_ERR_CUDA = 3,            /* CUDA runtime error, or no usable device */
     LS_ERR_CUFFT = 4,           /* cuFFT error */
     LS_ERR_UNSUPPORTED = 5,     /* size outside what the kernels index (n >= 2^31) */
-    LS_ERR_NOT_READY = 6        /* information requested before it exists */
+    LS_ERR_NOT_READY = 6,       /* information requested before it exists */
+    LS_ERR_TOO_LARGE = 7        /* size beyond the fixed scratch of a no-allocation entry point (LS_NOALLOC_MAX_ND) */
 };
 
 /* Stage indices for ls_get_stage_ms (CUDA-event timings of the last execute when opts.timing). */
@@ -234,6 +235,22 @@ int ls_direct_power(int64_t Nd, double f0, double df, int64_t k0, int64_t K, con
  * behaviour as ls_direct_power. */
 int ls_direct_sums(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
                    const void* dy, void* sums, void* cuda_stream);
+
+/* ls_direct_power_noalloc — ls_direct_power for callers that cannot allocate (code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc): same arguments, same kernels, same power, but the scratch (the
+ * statistics and 40 bytes per point) is a fixed device array inside the library instead of a cudaMalloc per call.
+ *   t, y, dy  device (on the CURRENT device), const double[Nd];   power  device, double[K] (written).
+ *   Nd <= LS_NOALLOC_MAX_ND, else LS_ERR_TOO_LARGE (nothing is enqueued).
+ * Calls no cudaMalloc / cudaFree and no allocating library routine; the first call on a device resolves the array's
+ * device address (cudaGetSymbolAddress: make that call before a capture starts).  ASYNCHRONOUS, unlike ls_direct_power:
+ * it enqueues one memset and three kernels on `cuda_stream` and returns; `power` is complete when the stream reaches
+ * that point.  The array (256 + 40 LS_NOALLOC_MAX_ND bytes = 2.6 MB) is held by every GPU that loads the library until
+ * the process exits, and is SHARED by all calls: calls that overlap on the GPU (two streams, two host threads) race on
+ * it — serialise them on one stream or with events.
+ * Errors: LS_ERR_INVALID_VALUE, LS_ERR_TOO_LARGE, LS_ERR_CUDA. */
+#define LS_NOALLOC_MAX_ND 65536
+int ls_direct_power_noalloc(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                            const void* dy, void* power, void* cuda_stream);
 
 const char* ls_strerror(int code);
 

@@ -15,7 +15,7 @@ __all__ = [
     "LS_F32", "LS_F64", "LS_OK", "STAGES", "LsError", "ls_opts", "lib_path", "load",
     "ls_plan", "ls_execute", "ls_execute_host", "ls_destroy", "ls_get_info", "ls_workspace_bytes", "ls_set_workspace",
     "ls_get_stage_ms", "ls_get_launch_counts", "ls_debug_modes", "ls_debug_stats", "ls_debug_points", "ls_debug_bins", "ls_debug_grid", "ls_debug_dinv",
-    "ls_debug_assemble", "ls_debug_guards", "ls_strerror", "ls_direct_power", "ls_direct_sums",
+    "ls_debug_assemble", "ls_debug_guards", "ls_strerror", "ls_direct_power", "ls_direct_sums", "ls_direct_power_noalloc",
     "exported_symbols", "Plan",
 ]
 
@@ -78,6 +78,7 @@ _SIGNATURES = {
                                     C.POINTER(C.c_double)]),
     "ls_direct_power": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
     "ls_direct_sums": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
+    "ls_direct_power_noalloc": (C.c_int, [C.c_int64, C.c_double, C.c_double, C.c_int64, C.c_int64] + [C.c_void_p] * 5),
     "ls_strerror": (C.c_char_p, [C.c_int]),
     "ls_destroy": (C.c_int, [C.c_void_p]),
 }
@@ -186,6 +187,20 @@ def ls_direct_sums(Nd, f0, df, k0, K, t, y, dy, sums, stream=0) -> None:
                                C.c_void_p(_ptr(dy)), C.c_void_p(_ptr(sums)), C.c_void_p(int(stream)))
     if rc != LS_OK:
         raise LsError(rc, "ls_direct_sums")
+
+
+LS_NOALLOC_MAX_ND = 65536
+LS_ERR_TOO_LARGE = 7
+
+
+def ls_direct_power_noalloc(Nd, f0, df, k0, K, t, y, dy, power, stream=0) -> None:
+    """ls_direct_power without any allocation (fixed scratch inside the library, Nd <= LS_NOALLOC_MAX_ND); asynchronous:
+    the caller synchronises the stream.  Calls that overlap on the GPU race on the shared scratch (ls.h)."""
+    rc = load().ls_direct_power_noalloc(int(Nd), float(f0), float(df), int(k0), int(K), C.c_void_p(_ptr(t)),
+                                        C.c_void_p(_ptr(y)), C.c_void_p(_ptr(dy)), C.c_void_p(_ptr(power)),
+                                        C.c_void_p(int(stream)))
+    if rc != LS_OK:
+        raise LsError(rc, "ls_direct_power_noalloc")
 
 
 def ls_get_stage_ms(plan) -> dict:

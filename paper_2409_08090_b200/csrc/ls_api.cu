@@ -313,6 +313,7 @@ const char* ls_strerror(int code) {
         case LS_ERR_CUFFT: return "cuFFT error";
         case LS_ERR_UNSUPPORTED: return "problem size not supported";
         case LS_ERR_NOT_READY: return "requested information is not available yet";
+        case LS_ERR_TOO_LARGE: return "size beyond the fixed scratch of a no-allocation entry point (Nd > LS_NOALLOC_MAX_ND)";
         default: return "unknown error code";
     }
 }

@@ -11,6 +11,8 @@
 // One thread owns kR consecutive frequencies: per point it seeds e^{2 pi i f t_j} at its first frequency
 // (phase by an FMA two-product of the double-double frequency, one sincospi) and winds it kR - 1 times by
 // the point's step phasor e^{2 pi i df t_j} (computed once per point by a preparation kernel).
+#include <mutex>
+
 #include "ls_internal.h"
 #include "ls_power.cuh"
 
@@ -173,4 +175,71 @@ extern "C" int ls_direct_sums(int64_t Nd, double f0, double df, int64_t k0, int6
                               const void* dy, void* sums, void* cuda_stream) {
     if (!sums) return LS_ERR_INVALID_VALUE;
     return direct_run(Nd, f0, df, k0, K, t, y, dy, nullptr, sums, cuda_stream);
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// ls_direct_power_noalloc — the same brute-force evaluation for callers that cannot allocate (code under CUDA graph
+// capture, tight serving loops, harnesses that forbid cudaMalloc).  The scratch of direct_run above — four sums and one
+// DirPoint per input point — lives in a file-scope device array of fixed size instead: 256 + 40 x LS_NOALLOC_MAX_ND bytes
+// (2.6 MB), held by every GPU that loads the library until the process exits.
+//
+// In host code `g_direct_scratch` is a host-side stand-in for the symbol, not a device address (a kernel given it
+// faults or, where the GPU can reach host memory, silently uses the wrong memory): the device address is resolved once per
+// device, with that device current, by cudaGetSymbolAddress, and that pointer is what the kernels get.
+//
+// Every call shares the array, which keeps the last call's contents: the sums are cleared on the stream first (the
+// points are overwritten before they are read).  Calls that overlap on the GPU (two streams, or two host threads) race.
+namespace lsb {
+namespace {
+constexpr size_t kNoAllocSumsBytes = 256;                       // four doubles, padded so that the points stay 256-aligned
+static __device__ __align__(256) unsigned char g_direct_scratch[kNoAllocSumsBytes + (size_t)LS_NOALLOC_MAX_ND * sizeof(DirPoint)];
+constexpr int kNoAllocMaxDevices = 64;
+unsigned char* g_direct_scratch_ptr[kNoAllocMaxDevices] = {nullptr};   // device address of the array, per device ordinal
+std::mutex g_direct_scratch_mu;
+
+// device address of the scratch on the CURRENT device (resolved on the first call per device; no allocation)
+int direct_scratch_on_current_device(unsigned char** out) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kNoAllocMaxDevices) {
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    std::lock_guard<std::mutex> lock(g_direct_scratch_mu);
+    if (!g_direct_scratch_ptr[dev]) {
+        void* ptr = nullptr;
+        if (cudaGetSymbolAddress(&ptr, g_direct_scratch) != cudaSuccess || !ptr) {
+            cudaGetLastError();
+            return LS_ERR_CUDA;
+        }
+        g_direct_scratch_ptr[dev] = (unsigned char*)ptr;
+    }
+    *out = g_direct_scratch_ptr[dev];
+    return LS_OK;
+}
+}  // namespace
+}  // namespace lsb
+
+extern "C" int ls_direct_power_noalloc(int64_t Nd, double f0, double df, int64_t k0, int64_t K, const void* t, const void* y,
+                                       const void* dy, void* power, void* cuda_stream) {
+    using namespace lsb;
+    if (Nd < 1 || K < 1 || k0 < 0 || !t || !y || !dy || !power || !(df > 0.0) || !(f0 >= 0.0)) return LS_ERR_INVALID_VALUE;
+    if (Nd > (int64_t)LS_NOALLOC_MAX_ND) return LS_ERR_TOO_LARGE;       // the fixed scratch holds LS_NOALLOC_MAX_ND points
+    unsigned char* base = nullptr;
+    const int rc = direct_scratch_on_current_device(&base);
+    if (rc != LS_OK) return rc;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    double* sums = reinterpret_cast<double*>(base);
+    DirPoint* pts = reinterpret_cast<DirPoint*>(base + kNoAllocSumsBytes);
+    if (cudaMemsetAsync(sums, 0, 4 * sizeof(double), s) != cudaSuccess) {      // the array keeps the last call's sums
+        cudaGetLastError();
+        return LS_ERR_CUDA;
+    }
+    const int nb = (int)std::min<long long>((Nd + 255) / 256, 1184);
+    ls_direct_stats_kernel<<<nb, 256, 0, s>>>((const double*)y, (const double*)dy, Nd, sums);
+    ls_direct_prepare_kernel<<<nb, 256, 0, s>>>((const double*)t, (const double*)y, (const double*)dy, Nd, df, sums, pts);
+    const long long threads = (K + kR - 1) / kR;
+    ls_direct_kernel<<<(unsigned)((threads + kDirThreads - 1) / kDirThreads), kDirThreads, 0, s>>>(pts, Nd, f0, df, k0, K, sums,
+                                                                                                 (double*)power, nullptr);
+    if (cudaGetLastError() != cudaSuccess) return LS_ERR_CUDA;
+    return LS_OK;
 }
