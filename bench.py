@@ -373,7 +373,7 @@ def run_ours(args):
         popts["upsampfac"] = info["n"] / w.Nf * (1 - 1e-12) if info["n"] & (info["n"] - 1) else 0.0   # same n as `plan`
     plan_t = None
     n5 = info["n"] % 5 == 0 and (info["n"] // 5) & (info["n"] // 5 - 1) == 0       # 5 x 2^k: own two-pass FFT, fused for batches
-    if popts["fft_impl"] == 2 or (popts["fft_impl"] == 0 and n5 and w.dtype == "f64"):
+    if popts["fft_impl"] == 2 or (popts["fft_impl"] == 0 and n5):
         try:
             plan_t = B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, ldt, w.batch, timing=1, no_autotune=1,
                             **dict(popts, fft_impl=3))
@@ -465,11 +465,11 @@ def run_ours(args):
     own_fft = ffts == 0
     L = args.tile_cells or (1024 if w.batch == 1 else 512)
     sbytes = stage_model_bytes(w, info, own_fft, L)
-    fused23 = own_fft and info["n"] >= 1 << 20 and stage["fft_pass3"] == 0.0 and stage["fft_pass2"] > 0.0
+    fused23 = own_fft and info["n"] >= 1 << 20 and stage["fft_pass3"] == 0.0 and stage["fft_pass2"] > 0.0 and w.dtype == "f64"
     if fused23:                                           # the library reports the fused kernel's time as pass 2
         stage["fft_pass23"] = stage.pop("fft_pass2")
         stage.pop("fft_pass3")
-    two_pass = own_fft and (info["n"] <= 65536 or n5)      # R1 x 256: there is no middle pass
+    two_pass = own_fft and (info["n"] <= 65536 or (n5 and info["n"] <= 5 << 16))      # R1 x 256: there is no middle pass
     fft_stages = ["fft_pass1", "fft_pass23"] if fused23 else ["fft_pass1", "fft_pass3"] if two_pass else ["fft_pass1", "fft_pass2", "fft_pass3"]
     own_stages = ["stats", "sort", "premul", "spread", "assemble"] + (fft_stages if own_fft else [])
     dom = max(own_stages, key=lambda k: stage[k])      # the dominant OWN kernel (cuFFT, when used, is a library)

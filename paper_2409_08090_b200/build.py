@@ -13,7 +13,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libls_b200.so")
-SOURCES = ["ls_api.cu", "ls_pre.cu", "ls_spread.cu", "ls_fft.cu", "ls_post.cu", "ls_direct.cu"]
+SOURCES = ["ls_api.cu", "ls_pre.cu", "ls_spread.cu", "ls_fft.cu", "ls_fft_f32.cu", "ls_post.cu", "ls_direct.cu"]
 HEADERS = [os.path.join(CSRC, "ls_internal.h"), os.path.join(CSRC, "ls_power.cuh"), os.path.join(HERE, "..", "include", "ls.h")]
 CUDA_HOME = os.environ.get("CUDA_HOME", "/usr/local/cuda")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

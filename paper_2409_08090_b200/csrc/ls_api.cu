@@ -421,6 +421,15 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         if (n5 && dtype == LS_F64 && !o.dy_per_series && o.fft_impl != 1 && !o.no_autotune && (double)n5 * ntrans * 16.0 > 64e6) {
             p->n = n5;
             auto5 = true;
+        } else if (dtype == LS_F32 && o.fft_impl != 1 && !o.no_autotune && ntrans <= 8 && [&] {
+                       // fp32, a few very long transforms (config 5): 5 x 2^k cells, k = 22 .. 25, where that lies between
+                       // 1.25 Nf and the power of two: the own three-pass transform (ls_fft_f32.cu) instead of cuFFT on a
+                       // 2,3,5-smooth size, and no zero fill of the empty tiles
+                       for (int k = 22; k <= 25; ++k)
+                           if ((double)(5LL << k) >= want && (5LL << k) < m) { p->n = 5LL << k; return true; }
+                       return false;
+                   }()) {
+            auto5 = true;
         } else
         if ((double)m > 1.6 * (double)Nf && (double)m * ntrans >= (double)((int64_t)1 << 20) && !o.no_autotune) {
             // the timed choice is cached per (Nf, dtype, transforms, device): the same arguments give the same grid — and
@@ -503,10 +512,10 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
     // bound by its 2-CTAs-per-SM arithmetic, by 1 % — so fusion is opt-in (fft_impl = 2), not the default.
     // ... except for batches on the 5 x 2^k grids: there the modes round trip (2 x 16 bytes per frequency and series) is the
     // largest item left and the fused pass reads its per-frequency terms from a table (config 4: 2.88 -> 2.45 ms)
-    p->fuse_assemble = p->own_fft && (o.fft_impl == 2 || (o.fft_impl == 0 && lsb::own_fft_rm5(p) && batch >= 8)) && !o.dy_per_series;
+    p->fuse_assemble = p->own_fft && dtype == LS_F64 && (o.fft_impl == 2 || (o.fft_impl == 0 && lsb::own_fft_rm5(p) && batch >= 8)) && !o.dy_per_series;
     // Passes 2 and 3 as one persistent kernel with the intermediate kept in L2 (ls_fft.cu): the default wherever
     // the pruned three-pass transform runs; fft_impl = 3 keeps the three separate launches (for comparison).
-    p->fuse_pass23 = p->fft_prune && !lsb::own_fft_rm5(p) && !p->fuse_assemble && o.fft_impl != 3;
+    p->fuse_pass23 = p->fft_prune && dtype == LS_F64 && !lsb::own_fft_rm5(p) && !p->fuse_assemble && o.fft_impl != 3;
 
     // double-double constants (host): n*df exactly, f_c = f0 + floor(Nf/2) df
     p->ndf = two_prod((double)p->n, df);
@@ -527,7 +536,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         if (p->own_fft) {
             if ((ce = dmalloc(p, (char**)&p->fft_wlo, (size_t)4096 * 16)) != cudaSuccess) break;
             if ((ce = dmalloc(p, (char**)&p->fft_whi, (size_t)std::max<int64_t>(4096, p->n / 4096) * 16)) != cudaSuccess) break;
-            p->modes_bytes = (size_t)p->slots * Nf * 16;
+            p->modes_bytes = (size_t)p->slots * Nf * 2 * B;
             if ((ce = dmalloc(p, (char**)&p->modes, p->modes_bytes)) != cudaSuccess) break;
             if (p->fuse_assemble && (ce = dmalloc(p, (char**)&p->ftab, (size_t)Nf * 32)) != cudaSuccess) break;
             if ((ce = lsb::own_fft_init(p, 0)) != cudaSuccess) break;
@@ -535,7 +544,7 @@ int ls_plan(ls_plan_t* out, int64_t Nd, int64_t Nf, double f0, double df, double
         // sums and both histograms live in ONE allocation so a single memset clears them per execute
         const size_t sums_bytes = ((size_t)batch * 4 * 8 + 255) & ~(size_t)255;
         const size_t hist_bytes = ((size_t)2 * p->nbins * 4 + 255) & ~(size_t)255;
-        const size_t mask_bytes = p->fft_prune ? (size_t)2 * (65536 / p->L) * 16 * 4 + 256 : (p->list_tiles ? 256 : 0);   // masks + 2 list counters
+        const size_t mask_bytes = p->fft_prune ? (size_t)2 * std::max(65536 / p->L, lsb::own_fft_ncoltiles(p)) * std::max(16, lsb::own_fft_rb(p)) * 4 + 256 : (p->list_tiles ? 256 : 0);   // masks + 2 list counters
         const size_t queue_bytes = p->fuse_pass23 ? (((size_t)(2 + 32 * p->slots) * 4 + 255) & ~(size_t)255) : 0;
         p->zeroed_bytes = sums_bytes + hist_bytes + mask_bytes + queue_bytes;
         if ((ce = dmalloc(p, (char**)&p->zeroed, p->zeroed_bytes)) != cudaSuccess) break;

@@ -994,21 +994,23 @@ int own_fft_rm5(const ls_plan_s* p) {                     // RM of the 5 x 2^k s
 bool own_fft_supported(const ls_plan_s* p) {
     const bool pow2 = (p->n & (p->n - 1)) == 0;
     if (p->dtype == LS_F64 && own_fft_rm5(p)) return true;
+    if (own_fft_f32_rm(p)) return true;                    // fp32, 5 x 2^22 .. 5 x 2^25 cells (ls_fft_f32.cu)
     if (p->dtype != LS_F64 || !pow2 || p->n < ((int64_t)1 << 12) || p->n > ((int64_t)1 << 24)) return false;
     return p->n < ((int64_t)1 << 20) || 65536 % p->L == 0;
 }
 bool own_fft_prunes(const ls_plan_s* p) { return p->n >= ((int64_t)1 << 20) || own_fft_rm5(p) != 0; }
 // spreading tiles per liveness-mask column: 65536 / L where the first pass works on rows of 65536 cells; 1 at the 5 x 2^k
 // sizes (rows of 256 cells: the masks are then one bit per TILE, word = tile % 32, bit = tile / 32 — at most 1280 tiles)
-int own_fft_ncoltiles(const ls_plan_s* p) { return own_fft_rm5(p) ? 1 : std::max(1, 65536 / p->L); }
+int own_fft_ncoltiles(const ls_plan_s* p) { return own_fft_rm5(p) ? 1 : own_fft_f32_rm(p) ? 131072 / p->L : std::max(1, 65536 / p->L); }
 // radix of the first pass / 16 where that pass is the 16 x RB kernel (n >= 2^20: R1 = n / 2^16; n <= 2^16: R1 = n / 2^8)
-int own_fft_rb(const ls_plan_s* p) { return own_fft_rm5(p) ? 32 : (int)(p->n >= ((int64_t)1 << 20) ? p->n >> 20 : p->n >> 12); }
+int own_fft_rb(const ls_plan_s* p) { return own_fft_rm5(p) ? 32 : own_fft_f32_rm(p) ? 5 * own_fft_f32_rm(p) / 2 : (int)(p->n >= ((int64_t)1 << 20) ? p->n >> 20 : p->n >> 12); }
 
 cudaError_t own_fft_init(ls_plan_s* p, cudaStream_t s) {
     const int cnt = (int)std::max<long long>(4096, p->n / 4096);
     ls_fft_tables_kernel<<<(cnt + 255) / 256, 256, 0, s>>>((double2*)p->fft_wlo, (double2*)p->fft_whi, p->n);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
+    if (p->dtype == LS_F32) return own_fft_f32_init(p, s);
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<16, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<8, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
     if ((e = cudaFuncSetAttribute(ls_fft_pass1_kernel<4, kPass1Threads>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kPass1Smem)) != cudaSuccess) return e;
@@ -1071,6 +1073,7 @@ static void fill_common(const ls_plan_s* p, FftArgs& a, int slot0, int n_x2) {
 // Pass 1 of transforms [slot0, slot0 + ntrans) of the plan's grids; the first n_x2 of them belong to the x2
 // point set (which liveness masks to prune by).
 cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s) {
+    if (p->dtype == LS_F32) return launch_own_fft_f32_pass1(p, slot0, ntrans, n_x2, s);
     FftArgs a;
     fill_common(p, a, slot0, n_x2);
     const long long inner1 = (long long)a.R2 * a.R3;       // 65536 (three passes) or 256 (two passes)
@@ -1108,6 +1111,7 @@ cudaError_t launch_own_fft_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, 
 }
 
 cudaError_t launch_own_fft_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
+    if (p->dtype == LS_F32) return launch_own_fft_f32_pass2(p, slot0, ntrans, s);
     FftArgs a;
     fill_common(p, a, slot0, 0);
     if (a.R2 == 1) return cudaSuccess;                     // two-pass sizes: nothing between pass 1 and the last pass
@@ -1166,6 +1170,7 @@ cudaError_t launch_own_fft_pass23(ls_plan_s* p, int slot0, int ntrans, cudaStrea
 // Pass 3 -> compact modes, transforms [slot0, slot0 + ntrans).
 cudaError_t launch_own_fft_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s) {
     if (ntrans <= 0) return cudaSuccess;
+    if (p->dtype == LS_F32) return launch_own_fft_f32_pass3(p, slot0, ntrans, s);
     FftArgs a;
     fill_common(p, a, slot0, 0);
     dim3 g3(a.R1 * a.R2 / kC, 1, ntrans);

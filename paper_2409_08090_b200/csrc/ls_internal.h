@@ -162,6 +162,12 @@ cudaError_t launch_tile_list(ls_plan_s* p, cudaStream_t s);
 cudaError_t launch_zero_list(ls_plan_s* p, int nrows_x2, int slot0_x2, int nrows_x1, int slot0_x1, int build_list, cudaStream_t s);
 // ---- ls_fft.cu: own FFT (fp64, n = 2^12 .. 2^24; first pass pruned and passes 2 + 3 fused from 2^20 on) ------
 bool own_fft_supported(const ls_plan_s* p);
+// ---- ls_fft_f32.cu: the own FFT for fp32 grids of 5 x 2^22 .. 5 x 2^25 cells (three passes 80 RM x 256 x 512)
+int own_fft_f32_rm(const ls_plan_s* p);           // RM of those sizes (fp32 plans only), else 0
+cudaError_t own_fft_f32_init(ls_plan_s* p, cudaStream_t s);
+cudaError_t launch_own_fft_f32_pass1(ls_plan_s* p, int slot0, int ntrans, int n_x2, cudaStream_t s);
+cudaError_t launch_own_fft_f32_pass2(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
+cudaError_t launch_own_fft_f32_pass3(ls_plan_s* p, int slot0, int ntrans, cudaStream_t s);
 int own_fft_rm5(const ls_plan_s* p);              // n = 5 x 2^k (two passes 80 RM x 256): RM, else 0
 bool own_fft_prunes(const ls_plan_s* p);          // first pass pruned by liveness masks (n >= 2^20)
 int own_fft_ncoltiles(const ls_plan_s* p);        // spreading tiles per liveness-mask column

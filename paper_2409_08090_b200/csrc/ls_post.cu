@@ -195,7 +195,7 @@ cudaError_t launch_debug_modes(ls_plan_s* p, int h_slot, int w_slot, int w2_slot
         ls_debug_modes_kernel<double><<<nb, 128, 0, s>>>(p->own_fft ? p->modes : p->grids, p->n, p->own_fft ? p->Nf : p->n, p->own_fft ? 1 : 0, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
                                                          K, (const long long*)d_kidx, d_out);
     else
-        ls_debug_modes_kernel<float><<<nb, 128, 0, s>>>(p->grids, p->n, p->n, 0, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
+        ls_debug_modes_kernel<float><<<nb, 128, 0, s>>>(p->own_fft ? p->modes : p->grids, p->n, p->own_fft ? p->Nf : p->n, p->own_fft ? 1 : 0, p->Nf / 2, p->dinv, h_slot, w_slot, w2_slot,
                                                         K, (const long long*)d_kidx, d_out);
     return cudaGetLastError();
 }

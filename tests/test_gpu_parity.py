@@ -292,9 +292,33 @@ def test_zero_fill_sweep_and_tile_lists_on_the_cufft_path():
     _check64(errors(gpu_power(ww, fft_impl=1, reserved=(2, 0))[0], oracle_power(ww)), pointwise=False)
 
 
+@pytest.mark.parametrize("k", [22, 23, 24])
+def test_own_fp32_fft_grids_of_5_times_a_power_of_two(k):
+    """fp32, n = 5 x 2^k (three passes 80 RM x 256 x 512, RM = 2, 4, 8; ls_fft_f32.cu; RM = 16 is config 5 itself, below):
+    clustered sampling as in config 5, so that most spreading tiles are empty and the first pass prunes; against cuFFT on
+    the same grid over the whole frequency grid and against the oracle on sampled k."""
+    n = 5 << k
+    w0 = scaled_workload(5, 150_000)
+    Nf = int(n / 1.3107)
+    w = _custom(w0.t, w0.y[0], w0.dy, w0.f0, w0.df, Nf, dtype="f32", eps=1e-5, name=f"f32_n5_{k}")
+    w.seed, w.injected = w0.seed, w0.injected
+    up = n / Nf * (1 - 1e-9)
+    P_own, ex = gpu_power(w, upsampfac=up, return_plan_info=True)
+    assert ex["info"]["n"] == n and ex["launches"][1] == 0
+    P_cu, exc = gpu_power(w, upsampfac=up, fft_impl=1, return_plan_info=True)
+    assert exc["info"]["n"] == n and exc["launches"][1] == 1
+    assert np.all(np.isfinite(P_own))
+    assert np.max(np.abs(P_own - P_cu)) / P_cu.max() <= 2e-5         # two fp32 FFTs of the same grids
+    ks = compare_indices(w, 300)
+    e = errors(P_own[0][ks], oracle_power(w, ks=ks))
+    assert e["Einf"] <= GATE_F32 and e["median"] <= 1e-4, e
+    assert abs(int(np.argmax(P_own[0])) - int(np.argmax(P_cu[0]))) <= 1
+
+
 def test_cfg5_full_size_fp32_sampled_frequencies():
     w = make_workload(5)
-    Pg = gpu_power(w)
+    Pg, ex = gpu_power(w, return_plan_info=True)
+    assert ex["info"]["n"] == 5 << 25 and ex["launches"][1] == 0       # the own fp32 transform (RM = 16), no cuFFT
     assert np.all(np.isfinite(Pg))
     ks = compare_indices(w, 256)                                       # SURVEY §8(d): K = 256 at config 5
     e = errors(Pg[0][ks], oracle_power(w, ks=ks))
