@@ -129,18 +129,27 @@ __constant__ float2 cW32[16];
 // Liveness: row l1 of column tile ct is bit (l1 / rb) of word [(set ncoltiles + ct) rb + l1 % rb], rb = J / 2 = R1 / 32,
 // so the 16 rows J i + j of a thread are bits 2 i + (j / rb) of ONE word.
 template <int RM>
-constexpr size_t pass1_smem() { return sizeof(float2) * (size_t)(80 * RM) * (kC1 + 1); }
+constexpr size_t pass1_smem() { return sizeof(float2) * ((size_t)16 * (5 * RM + 1) * kC1 + 80 * RM) + sizeof(double2) * 2 * kC1; }   // tile (padded) + table + column steps
 template <int RM>
 __global__ void __launch_bounds__(5 * RM * kC1, RM == 16 ? 2 : 1)
 ls_f32_pass1_kernel(const F32Args a) {
     constexpr int J = 5 * RM, R1 = 16 * J, RBW = J / 2;
+    // rows of 8 float2 = 64 bytes, J + 1 rows per ka: a warp's four consecutive ka then alternate between the two halves of
+    // the 128-byte bank line (with J rows they all start at bank 0: every access of stages 2 and 3 was a 2-way conflict)
+    constexpr int JP = J + 1;
     extern __shared__ __align__(16) unsigned char fsm[];
-    float2* S = reinterpret_cast<float2*>(fsm);              // [ka][j][c]
-    float2* wr = S + R1 * kC1;                               // w_R1^x, x < R1
+    float2* S = reinterpret_cast<float2*>(fsm);              // [ka][j (padded to JP)][c]
+    float2* wr = S + 16 * JP * kC1;                          // [ka][j] = w_R1^{ka j}: a warp's lookups are consecutive entries
     for (int x = threadIdx.x; x < R1; x += J * kC1) {
         double sn, cs;
-        sincospi(2.0 * (double)x / (double)R1, &sn, &cs);
+        sincospi(2.0 * (double)((x / J) * (x % J)) / (double)R1, &sn, &cs);
         wr[x] = make_float2((float)cs, (float)sn);
+    }
+    double2* colw = reinterpret_cast<double2*>(wr + R1);     // [2][kC1]: w_n^{J m}, w_n^{16 RM m} of the CTA's columns
+    if (threadIdx.x < 2 * kC1) {
+        const long long mc = (long long)blockIdx.x * kC1 + (threadIdx.x % kC1);
+        const long long e = (threadIdx.x < kC1 ? (long long)J : 16LL * RM) * mc;
+        sincospi(2.0 * (double)e / (double)a.n, &colw[threadIdx.x].y, &colw[threadIdx.x].x);
     }
     const int c = threadIdx.x % kC1, tj = threadIdx.x / kC1;
     const long long m = (long long)blockIdx.x * kC1 + c;     // column: 512 l2 + l3
@@ -164,7 +173,7 @@ ls_f32_pass1_kernel(const F32Args a) {
         fft16(x);
         __syncthreads();                                     // table ready
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) S[(ka * J + j) * kC1 + c] = cmul(x[pos16(ka)], wr[ka * j]);
+        for (int ka = 0; ka < 16; ++ka) S[(ka * JP + j) * kC1 + c] = cmul(x[pos16(ka)], wr[ka * J + j]);
     }
     __syncthreads();
 #pragma unroll
@@ -172,32 +181,39 @@ ls_f32_pass1_kernel(const F32Args a) {
         const int b = tj + J * r, ka = b & 15, q = b >> 4;
         float2 y[RM];
 #pragma unroll
-        for (int p = 0; p < RM; ++p) y[p] = S[(ka * J + 5 * p + q) * kC1 + c];
+        for (int p = 0; p < RM; ++p) y[p] = S[(ka * JP + 5 * p + q) * kC1 + c];
         fft_small<RM>(y);
 #pragma unroll
         for (int kp = 0; kp < RM; ++kp)
-            S[(ka * J + 5 * kp + q) * kC1 + c] = cmul(y[fft_pos<RM>(kp)], cTw5f[RM == 2 ? 0 : RM == 4 ? 1 : RM == 8 ? 2 : 3][q][kp]);
+            S[(ka * JP + 5 * kp + q) * kC1 + c] = cmul(y[fft_pos<RM>(kp)], cTw5f[RM == 2 ? 0 : RM == 4 ? 1 : RM == 8 ? 2 : 3][q][kp]);
     }
     __syncthreads();
+    // stage 3: butterfly b = ka + 16 kp = tj + J r (elements S[ka][5 kp + q]), outputs k1 = b + 16 RM kq times the inter-pass
+    // twiddle w_n^{k1 m} = w_n^{b m} (w_n^{16 RM m})^kq.  No table lookups: a warp's 32 gathered 16-byte entries cost the
+    // load/store unit as much as sixteen of its shared-memory accesses, and it is the unit this kernel is bound by.  The
+    // thread's base w_n^{tj m} is one double sincospi; its step over r, w_n^{J m}, and the step over kq, w_n^{16 RM m},
+    // depend on the column only and sit in shared memory (colw); the five-term chain over kq runs in fp32.
+    double2 twb;
+    sincospi(2.0 * (double)((long long)tj * m) / (double)a.n, &twb.y, &twb.x);
+    const double2 stb = colw[c];
+    const float2 st = to_f(colw[kC1 + c]);
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {                            // stage 3: butterfly (ka, kp), elements S[ka][5 kp + q]
+    for (int r = 0; r < 4; ++r) {
         const int b = tj + J * r;
         if (b < 16 * RM) {
             const int ka = b & 15, kp = b >> 4;
             float2 z[5];
 #pragma unroll
-            for (int q = 0; q < 5; ++q) z[q] = S[(ka * J + 5 * kp + q) * kC1 + c];
+            for (int q = 0; q < 5; ++q) z[q] = S[(ka * JP + 5 * kp + q) * kC1 + c];
             fft5(z);
-            // k1 = k0 + 16 RM kq, k0 = ka + 16 kp: w_n^{k1 m} = w_n^{k0 m} (w_n^{16 RM m})^kq, the chain in double
-            const unsigned mm = (unsigned)m;
-            double2 tw = twiddle_n(a, (unsigned)(ka + 16 * kp) * mm);
-            const double2 st = twiddle_n(a, (unsigned)(16 * RM) * mm);
+            float2 tw = to_f(twb);
 #pragma unroll
             for (int kq = 0; kq < 5; ++kq) {
-                base[(long long)(ka + 16 * (kp + RM * kq)) * kInner] = cmul(z[kq], to_f(tw));
-                tw = cmuld(tw, st);
+                base[(long long)(b + 16 * RM * kq) * kInner] = cmul(z[kq], tw);
+                tw = cmul(tw, st);
             }
         }
+        twb = cmuld(twb, stb);
     }
 }
 
@@ -259,9 +275,9 @@ ls_f32_pass3_kernel(const F32Args a) {
     extern __shared__ __align__(16) unsigned char fsm[];
     float2* S = reinterpret_cast<float2*>(fsm);              // [ka][jj][17]
     float2* w512 = S + 512 * (kC3 + 1);
-    for (int i = threadIdx.x; i < 512; i += 256) {
+    for (int i = threadIdx.x; i < 512; i += 256) {           // [ka][jj] = w_512^{ka jj}: consecutive entries per warp
         double sn, cs;
-        sincospi((double)i / 256.0, &sn, &cs);
+        sincospi((double)((i >> 5) * (i & 31)) / 256.0, &sn, &cs);
         w512[i] = make_float2((float)cs, (float)sn);
     }
     const int k1b = blockIdx.x * kC3, k2 = blockIdx.y, tr = blockIdx.z;
@@ -278,7 +294,7 @@ ls_f32_pass3_kernel(const F32Args a) {
             for (int i = 0; i < 16; ++i) x[i] = __ldcs(&row[32 * i + jj]);
             fft16(x);
 #pragma unroll
-            for (int ka = 0; ka < 16; ++ka) S[(ka * 32 + jj) * (kC3 + 1) + c] = cmul(x[pos16(ka)], w512[ka * jj]);
+            for (int ka = 0; ka < 16; ++ka) S[(ka * 32 + jj) * (kC3 + 1) + c] = cmul(x[pos16(ka)], w512[ka * 32 + jj]);
         }
     }
     __syncthreads();
