@@ -106,12 +106,14 @@ typedef struct {
                                stream): 0 = auto (on; off for good after three consecutive executes
                                with changed buffer pointers), 1 = never, 2 = always                 */
     int fft_impl;           /* 0 = auto: the library's own FFT where it exists (fp64 grids of 2^12..2^24 cells
-                               and of 5 x 2^13..5 x 2^16 cells; the powers of two below 2^20 not for large
-                               batches), else cuFFT.  For n >= 2^20 the own FFT is a pruned first pass plus ONE
+                               and of 5 x 2^13..5 x 2^16 cells, fp32 grids of 5 x 2^22..5 x 2^25 cells; the powers
+                               of two below 2^20 not for large batches), else cuFFT.  For n >= 2^20 the own FFT is a pruned first pass plus ONE
                                persistent kernel for passes 2 + 3 whose intermediate stays in L2.  A batch with
                                shared dy (upsampfac = 0, autotune on) takes a 5 x 2^k grid where one lies
                                between 1.25 Nf and the power of two: two passes, the first pruned, the last
-                               fused with the assembly.  1 = cuFFT plan.  2 = own FFT,
+                               fused with the assembly.  An fp32 plan of up to 8 transforms takes a grid of
+                               5 x 2^k cells, k = 22..25, where one lies in that range: three passes, the first
+                               pruned (ls_fft_f32.cu).  1 = cuFFT plan.  2 = own FFT,
                                three launches, the h transforms' last pass fused with deconvolution +
                                assembly.  3 = own FFT as three separate pass kernels and a separate
                                assembly (same arithmetic as auto; kept for comparison).  2 and 3 give
