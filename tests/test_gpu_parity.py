@@ -315,6 +315,47 @@ def test_own_fp32_fft_grids_of_5_times_a_power_of_two(k):
     assert abs(int(np.argmax(P_own[0])) - int(np.argmax(P_cu[0]))) <= 1
 
 
+def test_own_fp32_fft_batches_variants_and_mode_hook():
+    """The fp32 own-FFT path (n = 5 x 2^22) beyond one series: a batch of 3 with shared dy in one pass and in chunks of 2
+    (pass 1 reuses the liveness masks), per-series dy (M = 6), the fixed-mean pair of transforms, and the mode debug hook
+    on the compact fp32 mode array — each against the oracle on sampled k, the batch also against its single-series runs."""
+    import oracle
+    from oracle import variants
+    n = 5 << 22
+    w0 = scaled_workload(5, 60_000)
+    Nf = int(n / 1.3107)
+    up = n / Nf * (1 - 1e-9)
+    rng = np.random.default_rng(91)
+    y = np.stack([w0.y[0], 0.5 * w0.y[0] + 3.0, w0.y[0] + np.sin(2 * np.pi * w0.t / 2.7).astype(np.float32)])
+    wb = _custom(w0.t, y, w0.dy, w0.f0, w0.df, Nf, dtype="f32", eps=1e-5, name="f32_n5_batch")
+    wb.seed, wb.injected = w0.seed, w0.injected
+    ks = compare_indices(wb, 200)
+    P1, ex = gpu_power(wb, upsampfac=up, return_plan_info=True, debug_modes=(2, ks))
+    assert ex["info"]["n"] == n and ex["info"]["M"] == 5 and ex["launches"][1] == 0
+    P2 = gpu_power(wb, upsampfac=up, batch_chunk=2)
+    assert np.max(np.abs(P1 - P2)) <= 1e-6
+    for b in range(3):
+        e = errors(P1[b][ks], oracle_power(wb, b=b, ks=ks))
+        assert e["Einf"] <= GATE_F32 and e["median"] <= 1e-4, (b, e)
+    _, sums, _ = oracle.direct(wb.t, wb.y[2], wb.dy, wb.f0, wb.df, wb.Nf, k=ks, return_sums=True)
+    g = ex["modes"]
+    for a, b in ((0, 1), (2, 3), (4, 5)):                              # the three type-1 transforms, fp32: <~ eps
+        num = np.sqrt(np.sum((g[:, a] - sums[:, a]) ** 2 + (g[:, b] - sums[:, b]) ** 2))
+        assert num / np.sqrt(np.sum(sums[:, a] ** 2 + sums[:, b] ** 2)) <= 3e-5, (a, num)
+    wp = _custom(w0.t, y[:2], rng.uniform(0.5, 2.0, (2, w0.Nd)), w0.f0, w0.df, Nf, dtype="f32", eps=1e-5, name="f32_n5_per")
+    Pp, exp_ = gpu_power(wp, upsampfac=up, return_plan_info=True)
+    assert exp_["info"]["M"] == 6 and exp_["launches"][1] == 0
+    for b in range(2):
+        Po = oracle.direct(wp.t, wp.y[b], wp.dy[b], wp.f0, wp.df, wp.Nf, k=ks)
+        assert np.max(np.abs(Pp[b][ks] - Po)) / Po.max() <= GATE_F32, b
+    Pf, exf = gpu_power(wb, upsampfac=up, no_floating_mean=1, return_plan_info=True)
+    assert exf["info"]["M"] == 4 and exf["launches"][1] == 0
+    Pc = gpu_power(wb, upsampfac=up, no_floating_mean=1, fft_impl=1)   # same variant through cuFFT on the same grid
+    assert np.max(np.abs(Pf - Pc)) / Pc.max() <= 2e-5
+    Po = variants.power(wb.t, wb.y[1], wb.dy, wb.f0, wb.df, wb.Nf, k=ks, fit_mean=False)
+    assert np.max(np.abs(Pf[1][ks] - Po)) / Po.max() <= GATE_F32
+
+
 def test_cfg5_full_size_fp32_sampled_frequencies():
     w = make_workload(5)
     Pg, ex = gpu_power(w, return_plan_info=True)
