@@ -270,12 +270,14 @@ ls_f32_pass2_kernel(const F32Args a) {
 // (two 16-point ones and a radix-2 layer).  Output: mode k = k1 + R1 k2 + 256 R1 k3, stored at (k + half) mod n if that
 // is below Nf — the compact, centred layout the assembly kernel reads.
 constexpr size_t kPass3Smem = sizeof(float2) * (512 * (kC3 + 1) + 512);
-__global__ void __launch_bounds__(256, 2)      // three CTAs per SM (80 registers) measured slower: 1.70 against 1.61 ms
+// measured and not kept: three CTAs per SM at 80 registers (1.70 ms against 1.61), 32 rows per CTA for 256-byte output
+// runs (one 512-thread CTA per SM: 1.74 ms)
+__global__ void __launch_bounds__(16 * kC3, kC3 == 16 ? 2 : 1)
 ls_f32_pass3_kernel(const F32Args a) {
     extern __shared__ __align__(16) unsigned char fsm[];
     float2* S = reinterpret_cast<float2*>(fsm);              // [ka][jj][17]
     float2* w512 = S + 512 * (kC3 + 1);
-    for (int i = threadIdx.x; i < 512; i += 256) {           // [ka][jj] = w_512^{ka jj}: consecutive entries per warp
+    for (int i = threadIdx.x; i < 512; i += 16 * kC3) {      // [ka][jj] = w_512^{ka jj}: consecutive entries per warp
         double sn, cs;
         sincospi((double)((i >> 5) * (i & 31)) / 256.0, &sn, &cs);
         w512[i] = make_float2((float)cs, (float)sn);
@@ -286,20 +288,22 @@ ls_f32_pass3_kernel(const F32Args a) {
     {
         const int jl = threadIdx.x & 15, c = threadIdx.x >> 4;
         const float2* row = src + ((long long)(k1b + c) * 256 + k2) * 512;
+        float2 x0[16], x1[16];                               // all 32 loads in flight before the first butterfly
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-            const int jj = jl + 16 * h;
-            float2 x[16];
-#pragma unroll
-            for (int i = 0; i < 16; ++i) x[i] = __ldcs(&row[32 * i + jj]);
-            fft16(x);
-#pragma unroll
-            for (int ka = 0; ka < 16; ++ka) S[(ka * 32 + jj) * (kC3 + 1) + c] = cmul(x[pos16(ka)], w512[ka * 32 + jj]);
+        for (int i = 0; i < 16; ++i) {
+            x0[i] = __ldcs(&row[32 * i + jl]);
+            x1[i] = __ldcs(&row[32 * i + jl + 16]);
         }
+        fft16(x0);
+#pragma unroll
+        for (int ka = 0; ka < 16; ++ka) S[(ka * 32 + jl) * (kC3 + 1) + c] = cmul(x0[pos16(ka)], w512[ka * 32 + jl]);
+        fft16(x1);
+#pragma unroll
+        for (int ka = 0; ka < 16; ++ka) S[(ka * 32 + jl + 16) * (kC3 + 1) + c] = cmul(x1[pos16(ka)], w512[ka * 32 + jl + 16]);
     }
     __syncthreads();
     {
-        const int c = threadIdx.x & 15, ka = threadIdx.x >> 4;
+        const int c = threadIdx.x % kC3, ka = threadIdx.x / kC3;
         float2 e[16], o[16];
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
@@ -397,7 +401,7 @@ cudaError_t launch_own_fft_f32_pass3(ls_plan_s* p, int slot0, int ntrans, cudaSt
     if (ntrans <= 0) return cudaSuccess;
     F32Args a;
     fill_args(p, a, slot0, 0);
-    ls_f32_pass3_kernel<<<dim3(a.R1 / kC3, 256, ntrans), 256, kPass3Smem, s>>>(a);
+    ls_f32_pass3_kernel<<<dim3(a.R1 / kC3, 256, ntrans), 16 * kC3, kPass3Smem, s>>>(a);
     return cudaGetLastError();
 }
 
