@@ -37,38 +37,90 @@ struct F32Args {
     long long Nf, half;
 };
 
-__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
-__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
-__device__ __forceinline__ float2 cmul(float2 a, float2 w) { return make_float2(fmaf(a.x, w.x, -a.y * w.y), fmaf(a.x, w.y, a.y * w.x)); }
+// Complex arithmetic on Blackwell's packed fp32 pairs (add / sub / mul / fma .f32x2 -> FADD2, FMUL2, FFMA2): one
+// instruction per complex add and two per complex product instead of two and four.  The fp32 pipe does the same flops per
+// clock either way (measured: 72 - 74 TFLOP/s with FFMA and with FFMA2); what halves is the ISSUE slots, and these kernels
+// are issue-bound (profiles/r2_cfg5.md).  ptxas folds the packing moves, the (-y, x) swizzle of a multiplication by i and
+// the (x, x) broadcasts into operand modifiers.  Same roundings as the scalar forms.
+__device__ __forceinline__ unsigned long long pk(float2 a) {
+    unsigned long long r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a.x), "f"(a.y));
+    return r;
+}
+__device__ __forceinline__ float2 upk(unsigned long long r) {
+    float2 a;
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(a.x), "=f"(a.y) : "l"(r));
+    return a;
+}
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    unsigned long long d;
+    asm("add.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) {
+    unsigned long long d;
+    asm("sub.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+    unsigned long long d;
+    asm("mul.f32x2 %0, %1, %2;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)));
+    return upk(d);
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(pk(a)), "l"(pk(b)), "l"(pk(c)));
+    return upk(d);
+}
+// PK = false keeps the scalar forms: pass 2 runs at the DRAM roofline and was 5 % SLOWER with the packed ones (1.28 ms
+// against 1.22: more register-pair moves), passes 1 and 3 gained 8 % and 1 %.
+template <bool PK = true>
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) {
+    if constexpr (PK) return add2(a, b);
+    else return make_float2(a.x + b.x, a.y + b.y);
+}
+template <bool PK = true>
+__device__ __forceinline__ float2 csub(float2 a, float2 b) {
+    if constexpr (PK) return sub2(a, b);
+    else return make_float2(a.x - b.x, a.y - b.y);
+}
+// (a.x w.x - a.y w.y, a.x w.y + a.y w.x) = (a.x, a.x) (w.x, w.y) + (a.y, a.y) (-w.y, w.x)
+template <bool PK = true>
+__device__ __forceinline__ float2 cmul(float2 a, float2 w) {
+    if constexpr (PK) return fma2(make_float2(a.x, a.x), w, mul2(make_float2(a.y, a.y), make_float2(-w.y, w.x)));
+    else return make_float2(fmaf(a.x, w.x, -a.y * w.y), fmaf(a.x, w.y, a.y * w.x));
+}
 __device__ __forceinline__ float2 cmuli(float2 a) { return make_float2(-a.y, a.x); }
 __device__ __forceinline__ double2 cmuld(double2 a, double2 w) { return make_double2(fma(a.x, w.x, -a.y * w.y), fma(a.x, w.y, a.y * w.x)); }
 __device__ __forceinline__ float2 to_f(double2 w) { return make_float2((float)w.x, (float)w.y); }
 
 constexpr float kC1f = 0.92387953251128675613f, kS1f = 0.38268343236508977173f, kR2f = 0.70710678118654752440f;
 
+template <bool PK = true>
 __device__ __forceinline__ void fft4(float2& a, float2& b, float2& c, float2& d) {
-    const float2 t0 = cadd(a, c), t1 = csub(a, c), t2 = cadd(b, d), t3 = cmuli(csub(b, d));
-    a = cadd(t0, t2);
-    b = cadd(t1, t3);
-    c = csub(t0, t2);
-    d = csub(t1, t3);
+    const float2 t0 = cadd<PK>(a, c), t1 = csub<PK>(a, c), t2 = cadd<PK>(b, d), t3 = cmuli(csub<PK>(b, d));
+    a = cadd<PK>(t0, t2);
+    b = cadd<PK>(t1, t3);
+    c = csub<PK>(t0, t2);
+    d = csub<PK>(t1, t3);
 }
 // X_k = sum_l x_l e^{+2 pi i k l / 16}, in place; X_k ends at position pos16(k)
 __device__ __forceinline__ constexpr int pos16(int k) { return 4 * (k & 3) + (k >> 2); }
+template <bool PK = true>
 __device__ __forceinline__ void fft16(float2 (&x)[16]) {
 #pragma unroll
-    for (int b = 0; b < 4; ++b) fft4(x[b], x[4 + b], x[8 + b], x[12 + b]);
-    x[5] = cmul(x[5], make_float2(kC1f, kS1f));
-    x[6] = cmul(x[6], make_float2(kR2f, kR2f));
-    x[7] = cmul(x[7], make_float2(kS1f, kC1f));
-    x[9] = cmul(x[9], make_float2(kR2f, kR2f));
+    for (int b = 0; b < 4; ++b) fft4<PK>(x[b], x[4 + b], x[8 + b], x[12 + b]);
+    x[5] = cmul<PK>(x[5], make_float2(kC1f, kS1f));
+    x[6] = cmul<PK>(x[6], make_float2(kR2f, kR2f));
+    x[7] = cmul<PK>(x[7], make_float2(kS1f, kC1f));
+    x[9] = cmul<PK>(x[9], make_float2(kR2f, kR2f));
     x[10] = cmuli(x[10]);
-    x[11] = cmul(x[11], make_float2(-kR2f, kR2f));
-    x[13] = cmul(x[13], make_float2(kS1f, kC1f));
-    x[14] = cmul(x[14], make_float2(-kR2f, kR2f));
-    x[15] = cmul(x[15], make_float2(-kC1f, -kS1f));
+    x[11] = cmul<PK>(x[11], make_float2(-kR2f, kR2f));
+    x[13] = cmul<PK>(x[13], make_float2(kS1f, kC1f));
+    x[14] = cmul<PK>(x[14], make_float2(-kR2f, kR2f));
+    x[15] = cmul<PK>(x[15], make_float2(-kC1f, -kS1f));
 #pragma unroll
-    for (int ka = 0; ka < 4; ++ka) fft4(x[4 * ka], x[4 * ka + 1], x[4 * ka + 2], x[4 * ka + 3]);
+    for (int ka = 0; ka < 4; ++ka) fft4<PK>(x[4 * ka], x[4 * ka + 1], x[4 * ka + 2], x[4 * ka + 3]);
 }
 __device__ __forceinline__ void fft8(float2 (&x)[8]) {       // X_k at position 2 (k & 3) + (k >> 2)
     fft4(x[0], x[2], x[4], x[6]);
@@ -102,15 +154,17 @@ constexpr float kCos5a = 0.30901699437494742410f, kCos5b = -0.809016994374947424
 constexpr float kSin5a = 0.95105651629515357212f, kSin5b = 0.58778525229247312917f;
 __device__ __forceinline__ void fft5(float2 (&x)[5]) {       // natural order
     const float2 t1 = cadd(x[1], x[4]), t2 = cadd(x[2], x[3]), t3 = csub(x[1], x[4]), t4 = csub(x[2], x[3]);
-    const float2 a1 = make_float2(x[0].x + kCos5a * t1.x + kCos5b * t2.x, x[0].y + kCos5a * t1.y + kCos5b * t2.y);
-    const float2 a2 = make_float2(x[0].x + kCos5b * t1.x + kCos5a * t2.x, x[0].y + kCos5b * t1.y + kCos5a * t2.y);
-    const float2 b1 = make_float2(kSin5a * t3.x + kSin5b * t4.x, kSin5a * t3.y + kSin5b * t4.y);
-    const float2 b2 = make_float2(kSin5b * t3.x - kSin5a * t4.x, kSin5b * t3.y - kSin5a * t4.y);
-    x[0] = make_float2(x[0].x + t1.x + t2.x, x[0].y + t1.y + t2.y);
-    x[1] = make_float2(a1.x - b1.y, a1.y + b1.x);
-    x[4] = make_float2(a1.x + b1.y, a1.y - b1.x);
-    x[2] = make_float2(a2.x - b2.y, a2.y + b2.x);
-    x[3] = make_float2(a2.x + b2.y, a2.y - b2.x);
+    const float2 ca = make_float2(kCos5a, kCos5a), cb = make_float2(kCos5b, kCos5b);
+    const float2 sa = make_float2(kSin5a, kSin5a), sb = make_float2(kSin5b, kSin5b);
+    const float2 a1 = fma2(cb, t2, fma2(ca, t1, x[0]));
+    const float2 a2 = fma2(ca, t2, fma2(cb, t1, x[0]));
+    const float2 b1 = fma2(sb, t4, mul2(sa, t3));
+    const float2 b2 = fma2(sb, t3, mul2(make_float2(-kSin5a, -kSin5a), t4));
+    x[0] = cadd(x[0], cadd(t1, t2));
+    x[1] = cadd(a1, cmuli(b1));                          // a1 + i b1
+    x[4] = csub(a1, cmuli(b1));
+    x[2] = cadd(a2, cmuli(b2));
+    x[3] = csub(a2, cmuli(b2));
 }
 
 // w_n^e, e < n, in double from the two tables (e = 4096 e_hi + e_lo)
@@ -238,17 +292,17 @@ ls_f32_pass2_kernel(const F32Args a) {
         const int j = hi;
 #pragma unroll
         for (int i = 0; i < 16; ++i) x[i] = base[(16 * i + j) * 512];
-        fft16(x);
+        fft16<false>(x);
         __syncthreads();
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC2 + c] = cmul(x[pos16(ka)], w256[ka * 16 + j]);
+        for (int ka = 0; ka < 16; ++ka) Y[(ka * 16 + j) * kC2 + c] = cmul<false>(x[pos16(ka)], w256[ka * 16 + j]);
     }
     __syncthreads();
     {
         const int ka = hi;
 #pragma unroll
         for (int j = 0; j < 16; ++j) x[j] = Y[(ka * 16 + j) * kC2 + c];
-        fft16(x);
+        fft16<false>(x);
         // k2 = ka + 16 kb; exponent k2 l3 R1 < n; two interleaved chains (even / odd kb) in double
         const unsigned mm = (unsigned)m * (unsigned)a.R1;
         double2 tw = twiddle_n(a, (unsigned)ka * mm);
@@ -257,8 +311,8 @@ ls_f32_pass2_kernel(const F32Args a) {
         const double2 st2 = cmuld(st, st);
 #pragma unroll
         for (int kb = 0; kb < 16; kb += 2) {
-            base[(ka + 16 * kb) * 512] = cmul(x[pos16(kb)], to_f(tw));
-            base[(ka + 16 * kb + 16) * 512] = cmul(x[pos16(kb + 1)], to_f(tw1));
+            base[(ka + 16 * kb) * 512] = cmul<false>(x[pos16(kb)], to_f(tw));
+            base[(ka + 16 * kb + 16) * 512] = cmul<false>(x[pos16(kb + 1)], to_f(tw1));
             tw = cmuld(tw, st2);
             tw1 = cmuld(tw1, st2);
         }
