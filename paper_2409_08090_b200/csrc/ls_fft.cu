@@ -342,7 +342,7 @@ __device__ __forceinline__ void fft5(double2 (&x)[5]) {
 // work in a kernel that is bound by it.  [log2 RM - 1][q][kp], filled by own_fft_init.
 __constant__ double2 cTw5[4][5][16];
 template <int RM>
-constexpr size_t cols5_smem() { return sizeof(double2) * (size_t)(80 * RM) * (kC5 + 1); }   // tile + w_R1 table
+constexpr size_t cols5_smem() { return sizeof(double2) * ((size_t)(80 * RM) * (kC5 + 1) + 2 * kC5); }   // tile + w_R1 table + column steps
 template <int RM>
 __global__ void __launch_bounds__(5 * RM * kC5, 16 / RM)      // 640 threads per SM: two CTAs at RM = 8 need <= 102 registers
 ls_fft_cols5_kernel(const FftArgs a) {
@@ -354,6 +354,11 @@ ls_fft_cols5_kernel(const FftArgs a) {
         double sn, cs;
         sincospi(2.0 * (double)x / (double)R1, &sn, &cs);
         wr[x] = make_double2(cs, sn);
+    }
+    double2* colw = wr + R1;                                 // [2][kC5]: w_n^{J m}, w_n^{16 RM m} of the CTA's columns
+    if (threadIdx.x < 2 * kC5) {
+        const unsigned e = (unsigned)(threadIdx.x < kC5 ? J : 16 * RM) * (unsigned)(blockIdx.x * kC5 + threadIdx.x % kC5);
+        colw[threadIdx.x] = cmul(__ldg(&a.wlo[e & 4095u]), __ldg(&a.whi[e >> 12]));
     }
     const int c = threadIdx.x % kC5, tj = threadIdx.x / kC5;
     const int m = blockIdx.x * kC5 + c, tr = blockIdx.y;
@@ -388,8 +393,13 @@ ls_fft_cols5_kernel(const FftArgs a) {
             S[(ka * J + 5 * kp + q) * kC5 + c] = cmul(y[fft_pos<RM>(kp)], cTw5[RM == 2 ? 0 : RM == 4 ? 1 : RM == 8 ? 2 : 3][q][kp]);
     }
     __syncthreads();
+    // stage 3: butterfly b = ka + 16 kp = tj + J r (elements S[ka][5 kp + q]), outputs k1 = b + 16 RM kq times the inter-pass
+    // twiddle w_n^{k1 m} = w_n^{b m} (w_n^{16 RM m})^kq.  One table lookup per thread (w_n^{tj m}) instead of two per round: the
+    // step over r, w_n^{J m}, and the step over kq depend on the column only and come from shared memory (colw).
+    double2 twb = cmul(__ldg(&a.wlo[((unsigned)tj * (unsigned)m) & 4095u]), __ldg(&a.whi[((unsigned)tj * (unsigned)m) >> 12]));
+    const double2 stb = colw[c], st = colw[kC5 + c];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {                            // stage 3: butterfly (ka, kp), elements S[ka][5 kp + q]
+    for (int r = 0; r < 4; ++r) {
         const int b = tj + J * r;
         if (b < 16 * RM) {
             const int ka = b & 15, kp = b >> 4;
@@ -397,16 +407,14 @@ ls_fft_cols5_kernel(const FftArgs a) {
 #pragma unroll
             for (int q = 0; q < 5; ++q) z[q] = S[(ka * J + 5 * kp + q) * kC5 + c];
             fft5(z);
-            // k1 = k0 + 16 RM kq, k0 = ka + 16 kp: w_n^{k1 m} = w_n^{k0 m} (w_n^{16 RM m})^kq; both exponents < n
-            const unsigned e0 = (unsigned)(ka + 16 * kp) * (unsigned)m, es = (unsigned)(16 * RM) * (unsigned)m;
-            double2 tw = cmul(__ldg(&a.wlo[e0 & 4095u]), __ldg(&a.whi[e0 >> 12]));
-            const double2 st = cmul(__ldg(&a.wlo[es & 4095u]), __ldg(&a.whi[es >> 12]));
+            double2 tw = twb;
 #pragma unroll
             for (int kq = 0; kq < 5; ++kq) {
-                base[(long long)(ka + 16 * (kp + RM * kq)) * 256] = cmul(z[kq], tw);
+                base[(long long)(b + 16 * RM * kq) * 256] = cmul(z[kq], tw);
                 tw = cmul(tw, st);
             }
         }
+        twb = cmul(twb, stb);
     }
 }
 
