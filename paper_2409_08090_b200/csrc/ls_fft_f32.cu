@@ -331,9 +331,9 @@ ls_f32_pass3_kernel(const F32Args a) {
     extern __shared__ __align__(16) unsigned char fsm[];
     float2* S = reinterpret_cast<float2*>(fsm);              // [ka][jj][17]
     float2* w512 = S + 512 * (kC3 + 1);
-    for (int i = threadIdx.x; i < 512; i += 16 * kC3) {      // [ka][jj] = w_512^{ka jj}: consecutive entries per warp
+    for (int i = threadIdx.x; i < 512; i += 16 * kC3) {      // [ka][h][jl] = w_512^{ka (2 jl + h)}: consecutive entries per warp
         double sn, cs;
-        sincospi((double)((i >> 5) * (i & 31)) / 256.0, &sn, &cs);
+        sincospi((double)((i >> 5) * (2 * (i & 15) + ((i >> 4) & 1))) / 256.0, &sn, &cs);
         w512[i] = make_float2((float)cs, (float)sn);
     }
     const int k1b = blockIdx.x * kC3, k2 = blockIdx.y, tr = blockIdx.z;
@@ -342,11 +342,14 @@ ls_f32_pass3_kernel(const F32Args a) {
     {
         const int jl = threadIdx.x & 15, c = threadIdx.x >> 4;
         const float2* row = src + ((long long)(k1b + c) * 256 + k2) * 512;
-        float2 x0[16], x1[16];                               // all 32 loads in flight before the first butterfly
+        // the thread takes the adjacent columns jj = 2 jl and 2 jl + 1 of the 16 x 32 view: sixteen 16-byte loads; column
+        // jj is kept at position (jj & 1) 16 + (jj >> 1) of S, which is how the 32-point stage wants it (evens, then odds)
+        float2 x0[16], x1[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-            x0[i] = __ldcs(&row[32 * i + jl]);
-            x1[i] = __ldcs(&row[32 * i + jl + 16]);
+            const float4 v = __ldcs(reinterpret_cast<const float4*>(row) + 16 * i + jl);
+            x0[i] = make_float2(v.x, v.y);
+            x1[i] = make_float2(v.z, v.w);
         }
         fft16(x0);
 #pragma unroll
@@ -361,8 +364,8 @@ ls_f32_pass3_kernel(const F32Args a) {
         float2 e[16], o[16];
 #pragma unroll
         for (int q = 0; q < 16; ++q) {
-            e[q] = S[(ka * 32 + 2 * q) * (kC3 + 1) + c];
-            o[q] = S[(ka * 32 + 2 * q + 1) * (kC3 + 1) + c];
+            e[q] = S[(ka * 32 + q) * (kC3 + 1) + c];
+            o[q] = S[(ka * 32 + 16 + q) * (kC3 + 1) + c];
         }
         fft16(e);
         fft16(o);
