@@ -178,23 +178,26 @@ __constant__ float2 cTw5f[4][5][16];
 __constant__ float2 cW32[16];
 
 // Pass 1: radix R1 = 16 x RM x 5 over l1 (row stride 131 072 cells), one CTA = R1 rows x 8 columns held in shared memory
-// ([ka][j][c]) between the three stages, 5 RM threads per column.  l1 = J i + j (J = 5 RM), j = 5 p + q;
+// ([ka][j][c]) between the three stages, 5 RM thread rows x 4 column pairs.  l1 = J i + j (J = 5 RM), j = 5 p + q;
 // k1 = ka + 16 (kp + RM kq).  Same structure as ls_fft_cols5_kernel (ls_fft.cu), in fp32 and with a long row stride.
 // Liveness: row l1 of column tile ct is bit (l1 / rb) of word [(set ncoltiles + ct) rb + l1 % rb], rb = J / 2 = R1 / 32,
 // so the 16 rows J i + j of a thread are bits 2 i + (j / rb) of ONE word.
 template <int RM>
 constexpr size_t pass1_smem() { return sizeof(float2) * ((size_t)16 * (5 * RM + 1) * kC1 + 80 * RM) + sizeof(double2) * 2 * kC1; }   // tile (padded) + table + column steps
+// TWO adjacent columns per thread (5 RM x 4 threads per CTA): every shared-memory and global access is 16 bytes, the index
+// arithmetic and the stage twiddles are shared by the two columns (1.65 -> 1.61 ms at config 5 against one column per
+// thread; 16 columns per CTA for 128-byte row segments, one 640-thread CTA per SM: 1.70 ms).
 template <int RM>
-__global__ void __launch_bounds__(5 * RM * kC1, RM == 16 ? 2 : 1)
+__global__ void __launch_bounds__(5 * RM * (kC1 / 2), RM == 16 ? 2 : 1)
 ls_f32_pass1_kernel(const F32Args a) {
-    constexpr int J = 5 * RM, R1 = 16 * J, RBW = J / 2;
-    // rows of 8 float2 = 64 bytes, J + 1 rows per ka: a warp's four consecutive ka then alternate between the two halves of
-    // the 128-byte bank line (with J rows they all start at bank 0: every access of stages 2 and 3 was a 2-way conflict)
+    constexpr int J = 5 * RM, R1 = 16 * J, RBW = J / 2, NT = J * (kC1 / 2);
+    // rows of 8 float2 = 64 bytes, J + 1 rows per ka: a warp's consecutive ka then alternate between the two halves of the
+    // 128-byte bank line (with J rows they all start at bank 0: every access of stages 2 and 3 was a 2-way conflict)
     constexpr int JP = J + 1;
     extern __shared__ __align__(16) unsigned char fsm[];
     float2* S = reinterpret_cast<float2*>(fsm);              // [ka][j (padded to JP)][c]
     float2* wr = S + 16 * JP * kC1;                          // [ka][j] = w_R1^{ka j}: a warp's lookups are consecutive entries
-    for (int x = threadIdx.x; x < R1; x += J * kC1) {
+    for (int x = threadIdx.x; x < R1; x += NT) {
         double sn, cs;
         sincospi(2.0 * (double)((x / J) * (x % J)) / (double)R1, &sn, &cs);
         wr[x] = make_float2((float)cs, (float)sn);
@@ -205,10 +208,16 @@ ls_f32_pass1_kernel(const F32Args a) {
         const long long e = (threadIdx.x < kC1 ? (long long)J : 16LL * RM) * mc;
         sincospi(2.0 * (double)e / (double)a.n, &colw[threadIdx.x].y, &colw[threadIdx.x].x);
     }
-    const int c = threadIdx.x % kC1, tj = threadIdx.x / kC1;
-    const long long m = (long long)blockIdx.x * kC1 + c;     // column: 512 l2 + l3
+    const int c = 2 * (threadIdx.x % (kC1 / 2)), tj = threadIdx.x / (kC1 / 2);      // columns c, c + 1
+    const long long m = (long long)blockIdx.x * kC1 + c;
     const int tr = blockIdx.y;
     float2* base = a.grids + (long long)tr * a.n + m;
+    auto ld2 = [](const float2* p, float2& u, float2& v) {
+        const float4 q = *reinterpret_cast<const float4*>(p);
+        u = make_float2(q.x, q.y);
+        v = make_float2(q.z, q.w);
+    };
+    auto st2 = [](float2* p, float2 u, float2 v) { *reinterpret_cast<float4*>(p) = make_float4(u.x, u.y, v.x, v.y); };
     {
         const int j = tj;
         unsigned live = 0xffffffffu;
@@ -218,56 +227,67 @@ ls_f32_pass1_kernel(const F32Args a) {
             live = __ldg(&a.row_masks[((long long)set * a.ncoltiles + ct) * RBW + (j % RBW)]);
         }
         live >>= (j / RBW);
-        float2 x[16];
+        float2 x[16], y[16];
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
-            x[i] = make_float2(0.f, 0.f);
-            if ((live >> (2 * i)) & 1u) x[i] = base[(long long)(J * i + j) * kInner];
+            x[i] = y[i] = make_float2(0.f, 0.f);
+            if ((live >> (2 * i)) & 1u) ld2(base + (long long)(J * i + j) * kInner, x[i], y[i]);
         }
         fft16(x);
+        fft16(y);
         __syncthreads();                                     // table ready
 #pragma unroll
-        for (int ka = 0; ka < 16; ++ka) S[(ka * JP + j) * kC1 + c] = cmul(x[pos16(ka)], wr[ka * J + j]);
+        for (int ka = 0; ka < 16; ++ka) {
+            const float2 t = wr[ka * J + j];
+            st2(&S[(ka * JP + j) * kC1 + c], cmul(x[pos16(ka)], t), cmul(y[pos16(ka)], t));
+        }
     }
     __syncthreads();
 #pragma unroll
     for (int r = 0; r < 80 / J; ++r) {                       // stage 2: butterfly (ka, q), elements S[ka][5 p + q]
         const int b = tj + J * r, ka = b & 15, q = b >> 4;
-        float2 y[RM];
+        float2 u[RM], v[RM];
 #pragma unroll
-        for (int p = 0; p < RM; ++p) y[p] = S[(ka * JP + 5 * p + q) * kC1 + c];
-        fft_small<RM>(y);
+        for (int p = 0; p < RM; ++p) ld2(&S[(ka * JP + 5 * p + q) * kC1 + c], u[p], v[p]);
+        fft_small<RM>(u);
+        fft_small<RM>(v);
 #pragma unroll
-        for (int kp = 0; kp < RM; ++kp)
-            S[(ka * JP + 5 * kp + q) * kC1 + c] = cmul(y[fft_pos<RM>(kp)], cTw5f[RM == 2 ? 0 : RM == 4 ? 1 : RM == 8 ? 2 : 3][q][kp]);
+        for (int kp = 0; kp < RM; ++kp) {
+            const float2 t = cTw5f[RM == 2 ? 0 : RM == 4 ? 1 : RM == 8 ? 2 : 3][q][kp];
+            st2(&S[(ka * JP + 5 * kp + q) * kC1 + c], cmul(u[fft_pos<RM>(kp)], t), cmul(v[fft_pos<RM>(kp)], t));
+        }
     }
     __syncthreads();
     // stage 3: butterfly b = ka + 16 kp = tj + J r (elements S[ka][5 kp + q]), outputs k1 = b + 16 RM kq times the inter-pass
     // twiddle w_n^{k1 m} = w_n^{b m} (w_n^{16 RM m})^kq.  No table lookups: a warp's 32 gathered 16-byte entries cost the
-    // load/store unit as much as sixteen of its shared-memory accesses, and it is the unit this kernel is bound by.  The
-    // thread's base w_n^{tj m} is one double sincospi; its step over r, w_n^{J m}, and the step over kq, w_n^{16 RM m},
-    // depend on the column only and sit in shared memory (colw); the five-term chain over kq runs in fp32.
-    double2 twb;
-    sincospi(2.0 * (double)((long long)tj * m) / (double)a.n, &twb.y, &twb.x);
-    const double2 stb = colw[c];
-    const float2 st = to_f(colw[kC1 + c]);
+    // load/store unit as much as sixteen of its shared-memory accesses.  Per column the base w_n^{tj m} is one double
+    // sincospi; its step over r, w_n^{J m}, and the step over kq, w_n^{16 RM m}, depend on the column only and sit in shared
+    // memory (colw); the five-term chain over kq runs in fp32.
+    double2 twb0, twb1;
+    sincospi(2.0 * (double)((long long)tj * m) / (double)a.n, &twb0.y, &twb0.x);
+    sincospi(2.0 * (double)((long long)tj * (m + 1)) / (double)a.n, &twb1.y, &twb1.x);
+    const double2 stb0 = colw[c], stb1 = colw[c + 1];
+    const float2 sq0 = to_f(colw[kC1 + c]), sq1 = to_f(colw[kC1 + c + 1]);
 #pragma unroll
     for (int r = 0; r < 4; ++r) {
         const int b = tj + J * r;
         if (b < 16 * RM) {
             const int ka = b & 15, kp = b >> 4;
-            float2 z[5];
+            float2 z0[5], z1[5];
 #pragma unroll
-            for (int q = 0; q < 5; ++q) z[q] = S[(ka * JP + 5 * kp + q) * kC1 + c];
-            fft5(z);
-            float2 tw = to_f(twb);
+            for (int q = 0; q < 5; ++q) ld2(&S[(ka * JP + 5 * kp + q) * kC1 + c], z0[q], z1[q]);
+            fft5(z0);
+            fft5(z1);
+            float2 t0 = to_f(twb0), t1 = to_f(twb1);
 #pragma unroll
             for (int kq = 0; kq < 5; ++kq) {
-                base[(long long)(b + 16 * RM * kq) * kInner] = cmul(z[kq], tw);
-                tw = cmul(tw, st);
+                st2(base + (long long)(b + 16 * RM * kq) * kInner, cmul(z0[kq], t0), cmul(z1[kq], t1));
+                t0 = cmul(t0, sq0);
+                t1 = cmul(t1, sq1);
             }
         }
-        twb = cmuld(twb, stb);
+        twb0 = cmuld(twb0, stb0);
+        twb1 = cmuld(twb1, stb1);
     }
 }
 
@@ -439,10 +459,10 @@ cudaError_t launch_own_fft_f32_pass1(ls_plan_s* p, int slot0, int ntrans, int n_
     fill_args(p, a, slot0, n_x2);
     const dim3 g((unsigned)(kInner / kC1), ntrans);
     switch (own_fft_f32_rm(p)) {
-        case 2: ls_f32_pass1_kernel<2><<<g, 5 * 2 * kC1, pass1_smem<2>(), s>>>(a); break;
-        case 4: ls_f32_pass1_kernel<4><<<g, 5 * 4 * kC1, pass1_smem<4>(), s>>>(a); break;
-        case 8: ls_f32_pass1_kernel<8><<<g, 5 * 8 * kC1, pass1_smem<8>(), s>>>(a); break;
-        default: ls_f32_pass1_kernel<16><<<g, 5 * 16 * kC1, pass1_smem<16>(), s>>>(a); break;
+        case 2: ls_f32_pass1_kernel<2><<<g, 5 * 2 * kC1 / 2, pass1_smem<2>(), s>>>(a); break;
+        case 4: ls_f32_pass1_kernel<4><<<g, 5 * 4 * kC1 / 2, pass1_smem<4>(), s>>>(a); break;
+        case 8: ls_f32_pass1_kernel<8><<<g, 5 * 8 * kC1 / 2, pass1_smem<8>(), s>>>(a); break;
+        default: ls_f32_pass1_kernel<16><<<g, 5 * 16 * kC1 / 2, pass1_smem<16>(), s>>>(a); break;
     }
     return cudaGetLastError();
 }
