@@ -115,7 +115,7 @@ typedef struct {
                                5 x 2^k cells, k = 22..25, where one lies in that range: three passes, the first
                                pruned (ls_fft_f32.cu).  1 = cuFFT plan.  2 = own FFT,
                                three launches, the h transforms' last pass fused with deconvolution +
-                               assembly.  3 = own FFT as three separate pass kernels and a separate
+                               assembly (fp64 with shared dy; otherwise the same as 3).  3 = own FFT as three separate pass kernels and a separate
                                assembly (same arithmetic as auto; kept for comparison).  2 and 3 give
                                LS_ERR_UNSUPPORTED where the own FFT does not exist                   */
     int no_floating_mean;   /* 0: floating mean, six sums (default; north_star).  1: the fixed-mean form of
