@@ -11,7 +11,7 @@ from paper_2409_08090_b200.workloads import Workload, make_workload, scaled_work
 pytestmark = pytest.mark.gpu
 
 
-def _run(w, monkeypatch, host=False, repeat=2, **opts):
+def _run(w, monkeypatch, host=False, repeat=2, expect=None, **opts):
     torch = require_cuda()
     from paper_2409_08090_b200 import binding as B
     monkeypatch.setenv("LS_B200_GUARD", "1")
@@ -20,6 +20,8 @@ def _run(w, monkeypatch, host=False, repeat=2, **opts):
     per = 1 if w.dy.ndim == 2 else 0
     with B.Plan(w.Nd, w.Nf, w.f0, w.df, w.eps, B.LS_F64 if w.dtype == "f64" else B.LS_F32, w.batch, dy_per_series=per, **opts) as plan:
         s = torch.cuda.Stream()
+        if expect is not None:                       # (n, cuFFT execs per execute) the case is meant to exercise
+            assert plan.info["n"] == expect[0], plan.info
         if host:
             P = np.empty((w.batch, w.Nf), dtype=w.np_dtype)
             for _ in range(repeat):
@@ -32,6 +34,8 @@ def _run(w, monkeypatch, host=False, repeat=2, **opts):
                 plan.execute(t, y, dy, P, s.cuda_stream)
             torch.cuda.synchronize()
             assert bool(torch.isfinite(P).all())
+        if expect is not None:
+            assert plan.launch_counts()[1] == expect[1]
         return B.ls_debug_guards(plan.handle)
 
 
@@ -42,6 +46,10 @@ def _p20(batch=1):
     df = 1.0 / (5 * (t.max() - t.min()))
     y = np.stack([np.sin(2 * np.pi * 3.3 * t + b) + rng.normal(0, 1, Nd) for b in range(batch)])
     return Workload("guards_p20", t, y, dy, df, df, Nf, "f64", 1e-9)
+
+
+def _resized(w, Nf):
+    return Workload(w.name + "_resized", w.t, w.y, w.dy, w.f0, w.df, Nf, w.dtype, w.eps)
 
 
 def test_no_kernel_writes_outside_its_buffers(monkeypatch):
@@ -58,6 +66,16 @@ def test_no_kernel_writes_outside_its_buffers(monkeypatch):
     assert _run(w4, monkeypatch, no_floating_mean=1) == 0                           # fixed mean: shorter slot layout
     assert _run(scaled_workload(5, 60_000), monkeypatch) == 0                       # fp32, clustered
     assert _run(scaled_workload(5, 60_000), monkeypatch, t_is_dtype=0, tile_cells=256) == 0
+    # the round-2 transforms on grids of 5 x 2^k cells: fp64 two passes (a batch: pruned first pass, fused last pass; and
+    # one series through the unfused kernels), fp32 three passes (pruned first pass, liveness masks of 2 x 128 x 5 words)
+    w5 = scaled_workload(4, 1500, batch=9)
+    n5 = 5 << 13
+    assert _run(_resized(w5, int(n5 / 1.3107)), monkeypatch, expect=(n5, 0), upsampfac=n5 / int(n5 / 1.3107) * (1 - 1e-9)) == 0
+    assert _run(_resized(scaled_workload(2, 3000), int((5 << 14) / 1.3107)), monkeypatch, expect=(5 << 14, 0), fft_impl=3,
+                upsampfac=(5 << 14) / int((5 << 14) / 1.3107) * (1 - 1e-9)) == 0
+    wf = scaled_workload(5, 60_000)
+    nf = 5 << 22
+    assert _run(_resized(wf, int(nf / 1.3107)), monkeypatch, expect=(nf, 0), upsampfac=nf / int(nf / 1.3107) * (1 - 1e-9), tile_cells=512) == 0
 
 
 def test_guards_need_the_environment_variable(monkeypatch):
